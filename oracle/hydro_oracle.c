@@ -1,0 +1,495 @@
+/*
+ * oracle/hydro_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, obviously-correct CPU statement of the hot path that
+ * BASELINE.json:north_star names: one unsplit method-of-lines compressible
+ * hydro advance (gamma-law EOS, PPM with the Colella-Woodward limiter, HLLC on
+ * every x/y/z face, flux divergence + constant gravity, SSP-RK2, ghost fill,
+ * CFL reduction) of a Castro-style state on a uniform-level MultiFab of boxes
+ * with ghost zones (sec. II, MultiFab/Fab/Box; sec. III,
+ * "a slope ... calculated by looking at several zones to the left and right"
+ * feeding "a polynomial approximation of the fluid state").
+ *
+ * The paper prints no equations (SURVEY.md header), so every step follows
+ * SURVEY.md sec. 8(c) O1..O9 and readings S1..S22 (restated in DESIGN.md).  Each
+ * function below cites the step it implements.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load this file.  It shares no code, header, table or
+ * helper with paper_2007_05218_b200/csrc (the CUDA path); neither includes the
+ * other.
+ *
+ * Floating-point contract (S18): FP64, every expression evaluated as written,
+ * one IEEE operation per operator, no FMA contraction (compile with
+ * -ffp-contract=off), constants HALF = 0.5, SIXTH = 1.0/6.0, dxinv = 1.0/dx
+ * used as multipliers.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): P1 free-stream, P2 conservation,
+ * P3 Sod exact solution, P4 Sedov radius, P5 PPM worked example (exact
+ * rationals), P6 HLLC worked example, P7 axis permutation, P8 decomposition
+ * invariance, P9 3-D = 1-D, P10 gravity closed form, P11 dt closed form, P12
+ * ghost fill on index-encoded data, P13 order of accuracy.
+ * Parity unpinned: behaviour when the small_dens / small_pres floors trigger
+ * (exercised GPU-vs-oracle only).
+ *
+ * State layout (a1): SoA FP64, idx = (((b*NVAR + c)*NZt + k)*NYt + j)*NXt + i,
+ * b = (bk*NBy + bj)*NBx + bi, valid zone (i,j,k) at padded (i+NG, j+NG, k+NG).
+ * Components: 0 rho, 1 rho*u, 2 rho*v, 3 rho*w, 4 rho*E, 5 rho*e, 6.. rho*X_k.
+ * Flux/conserved components (NFLUX = 5+nspec): the above without rho*e, i.e.
+ * flux slot f maps to state component (f < 5 ? f : f+1).
+ * Primitives (NQ = 5+nspec): 0 rho, 1 u, 2 v, 3 w, 4 p, 5.. X_k.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define HALF 0.5
+static const double SIXTH = 1.0 / 6.0;
+
+typedef struct {
+    int32_t ndom[3];
+    int32_t nbox[3];
+    int32_t ng;
+    int32_t nspec;
+    int32_t bc_lo[3], bc_hi[3]; /* 0 periodic, 1 outflow, 2 reflect */
+    double prob_lo[3], prob_hi[3];
+    double gamma, cfl;
+    double grav[3];
+    double small_dens, small_pres;
+} oracle_params;
+
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2 };
+
+static double dmin(double a, double b) { return a < b ? a : b; }
+static double dmax(double a, double b) { return a > b ? a : b; }
+
+/* ---- geometry helpers ---------------------------------------------------- */
+typedef struct {
+    int nvar, nflux, nq, ng;
+    int nb[3];   /* valid zones per box            */
+    int nt[3];   /* padded zones per box           */
+    int NB[3];   /* boxes per dimension            */
+    int nboxes;
+    size_t comp_stride; /* doubles per (box, component) */
+    size_t box_stride;  /* doubles per box              */
+    double dx[3], dxinv[3];
+} geom_t;
+
+static int make_geom(const oracle_params *p, geom_t *g)
+{
+    if (!p) return -1;
+    if (p->ng < 3 || p->nspec < 0) return -1;
+    g->nvar = 6 + p->nspec;
+    g->nflux = 5 + p->nspec;
+    g->nq = 5 + p->nspec;
+    g->ng = p->ng;
+    g->nboxes = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (p->ndom[d] <= 0 || p->nbox[d] <= 0) return -1;
+        if (p->ndom[d] % p->nbox[d] != 0) return -1;
+        if ((p->bc_lo[d] == BC_PERIODIC) != (p->bc_hi[d] == BC_PERIODIC)) return -1;
+        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 2 || p->bc_hi[d] < 0 || p->bc_hi[d] > 2) return -1;
+        g->nb[d] = p->nbox[d];
+        g->nt[d] = p->nbox[d] + 2 * p->ng;
+        g->NB[d] = p->ndom[d] / p->nbox[d];
+        g->nboxes *= g->NB[d];
+        g->dx[d] = (p->prob_hi[d] - p->prob_lo[d]) / p->ndom[d];
+        g->dxinv[d] = 1.0 / g->dx[d];
+    }
+    g->comp_stride = (size_t)g->nt[0] * g->nt[1] * g->nt[2];
+    g->box_stride = g->comp_stride * g->nvar;
+    return 0;
+}
+
+static size_t zidx(const geom_t *g, int i, int j, int k) /* padded indices */
+{
+    return ((size_t)k * g->nt[1] + j) * g->nt[0] + i;
+}
+
+size_t oracle_state_doubles(const oracle_params *p)
+{
+    geom_t g;
+    if (make_geom(p, &g)) return 0;
+    return g.box_stride * (size_t)g.nboxes;
+}
+
+/* ---- O1 ghost fill --------------------------------- */
+/* Maps a global index along dimension d to the valid global index that
+ * supplies it, and reports whether a reflecting wall was crossed. */
+static int map_global(const oracle_params *p, int d, int gidx, int *sgn)
+{
+    int n = p->ndom[d];
+    *sgn = 1;
+    if (gidx >= 0 && gidx < n) return gidx;
+    int bc = gidx < 0 ? p->bc_lo[d] : p->bc_hi[d];
+    if (bc == BC_PERIODIC) return ((gidx % n) + n) % n;
+    if (bc == BC_OUTFLOW) return gidx < 0 ? 0 : n - 1;
+    /* reflect */
+    *sgn = -1;
+    return gidx < 0 ? -1 - gidx : 2 * n - 1 - gidx;
+}
+
+int oracle_fill_ghosts(const oracle_params *p, double *U)
+{
+    geom_t g;
+    if (make_geom(p, &g) || !U) return -1;
+    const int ng = g.ng;
+    for (int bk = 0; bk < g.NB[2]; ++bk)
+    for (int bj = 0; bj < g.NB[1]; ++bj)
+    for (int bi = 0; bi < g.NB[0]; ++bi) {
+        size_t b = ((size_t)bk * g.NB[1] + bj) * g.NB[0] + bi;
+        for (int kl = 0; kl < g.nt[2]; ++kl)
+        for (int jl = 0; jl < g.nt[1]; ++jl)
+        for (int il = 0; il < g.nt[0]; ++il) {
+            int valid = il >= ng && il < ng + g.nb[0] && jl >= ng && jl < ng + g.nb[1] &&
+                        kl >= ng && kl < ng + g.nb[2];
+            if (valid) continue;
+            int sg[3];
+            int gx = map_global(p, 0, bi * g.nb[0] + il - ng, &sg[0]);
+            int gy = map_global(p, 1, bj * g.nb[1] + jl - ng, &sg[1]);
+            int gz = map_global(p, 2, bk * g.nb[2] + kl - ng, &sg[2]);
+            size_t sb = ((size_t)(gz / g.nb[2]) * g.NB[1] + gy / g.nb[1]) * g.NB[0] + gx / g.nb[0];
+            size_t sz = zidx(&g, gx % g.nb[0] + ng, gy % g.nb[1] + ng, gz % g.nb[2] + ng);
+            size_t dz = zidx(&g, il, jl, kl);
+            for (int c = 0; c < g.nvar; ++c) {
+                double v = U[sb * g.box_stride + c * g.comp_stride + sz];
+                if (c >= 1 && c <= 3 && sg[c - 1] < 0) v = -v;
+                U[b * g.box_stride + c * g.comp_stride + dz] = v;
+            }
+        }
+    }
+    return 0;
+}
+
+/* ---- O2 primitives -------------------------------------- */
+/* Uc: NVAR conserved values of one zone; q: NQ primitives out. */
+void oracle_cons_to_prim(double gamma, double small_dens, double small_pres, int nspec,
+                         const double *Uc, double *q)
+{
+    double rho = dmax(Uc[0], small_dens);
+    double rinv = 1.0 / rho;
+    q[0] = rho;
+    q[1] = Uc[1] * rinv;
+    q[2] = Uc[2] * rinv;
+    q[3] = Uc[3] * rinv;
+    q[4] = dmax((gamma - 1.0) * Uc[5], small_pres);
+    for (int s = 0; s < nspec; ++s) q[5 + s] = Uc[6 + s] * rinv;
+}
+
+/* ---- O3 + O4 PPM along one line (CW84 eqs. 1.6-1.8, 1.10) ---------------- */
+/* a[0..n-1] zone averages.  Outputs (arrays of length n):
+ *   s[i]   limited slope of zone i,                 valid for i = 1..n-2
+ *   e[i]   edge value between zones i and i+1,      valid for i = 1..n-3
+ *   aL[i], aR[i] monotonised parabola edges of zone i, valid for i = 2..n-3
+ * Entries outside the valid ranges are set to 0. */
+void oracle_ppm_line(const double *a, int n, double *s, double *e, double *aL, double *aR)
+{
+    for (int i = 0; i < n; ++i) { s[i] = 0.0; e[i] = 0.0; aL[i] = 0.0; aR[i] = 0.0; }
+    for (int i = 1; i <= n - 2; ++i) {
+        double dp = a[i + 1] - a[i];
+        double dm = a[i] - a[i - 1];
+        double dc = HALF * (a[i + 1] - a[i - 1]);
+        if (dp * dm > 0.0) {
+            double lim = dmin(fabs(dc), dmin(2.0 * fabs(dp), 2.0 * fabs(dm)));
+            s[i] = copysign(lim, dc);
+        } else {
+            s[i] = 0.0;
+        }
+    }
+    for (int i = 1; i <= n - 3; ++i)
+        e[i] = a[i] + HALF * (a[i + 1] - a[i]) - SIXTH * (s[i + 1] - s[i]);
+    for (int i = 2; i <= n - 3; ++i) {
+        double l = e[i - 1], r = e[i], ac = a[i];
+        if ((r - ac) * (ac - l) <= 0.0) {
+            l = ac;
+            r = ac;
+        } else {
+            double d = r - l;
+            double m = ac - HALF * (l + r);
+            double t = d * d * SIXTH;
+            if (d * m > t) l = 3.0 * ac - 2.0 * r;
+            else if (-t > d * m) r = 3.0 * ac - 2.0 * l;
+        }
+        aL[i] = l;
+        aR[i] = r;
+    }
+}
+
+/* ---- O5 HLLC (Toro star-state form, Davis wave speeds; S6, S7, S8) ------- */
+/* dir: 0,1,2.  qL, qR: NQ primitives of the left/right face states.
+ * F: NFLUX fluxes out (rho, rho*u, rho*v, rho*w, rho*E, rho*X_k). */
+void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, int nspec,
+                 const double *qL, const double *qR, double *F)
+{
+    const double gm1inv = 1.0 / (gamma - 1.0);
+    double rK[2], vK[2][3], pK[2], nK[2], rinvK[2], cK[2], EK[2], FK[2][5], UK[2][5];
+    const double *q[2] = { qL, qR };
+    for (int K = 0; K < 2; ++K) {
+        rK[K] = dmax(q[K][0], small_dens);
+        pK[K] = dmax(q[K][4], small_pres);
+        vK[K][0] = q[K][1]; vK[K][1] = q[K][2]; vK[K][2] = q[K][3];
+        nK[K] = vK[K][dir];
+        rinvK[K] = 1.0 / rK[K];
+        cK[K] = sqrt(gamma * pK[K] * rinvK[K]);
+        EK[K] = pK[K] * gm1inv +
+                HALF * rK[K] * (vK[K][0] * vK[K][0] + vK[K][1] * vK[K][1] + vK[K][2] * vK[K][2]);
+        FK[K][0] = rK[K] * nK[K];
+        for (int c = 0; c < 3; ++c) {
+            FK[K][1 + c] = rK[K] * nK[K] * vK[K][c];
+            if (c == dir) FK[K][1 + c] = FK[K][1 + c] + pK[K];
+        }
+        FK[K][4] = (EK[K] + pK[K]) * nK[K];
+        UK[K][0] = rK[K];
+        for (int c = 0; c < 3; ++c) UK[K][1 + c] = rK[K] * vK[K][c];
+        UK[K][4] = EK[K];
+    }
+    double SL = dmin(nK[0] - cK[0], nK[1] - cK[1]);
+    double SR = dmax(nK[0] + cK[0], nK[1] + cK[1]);
+    if (SL >= 0.0) {
+        for (int c = 0; c < 5; ++c) F[c] = FK[0][c];
+    } else if (SR <= 0.0) {
+        for (int c = 0; c < 5; ++c) F[c] = FK[1][c];
+    } else {
+        double mL = rK[0] * (SL - nK[0]);
+        double mR = rK[1] * (SR - nK[1]);
+        double SM = (pK[1] - pK[0] + mL * nK[0] - mR * nK[1]) / (mL - mR);
+        int K = SM >= 0.0 ? 0 : 1;
+        double S = K == 0 ? SL : SR;
+        double mK = K == 0 ? mL : mR;
+        double fac = mK / (S - SM);
+        double Us[5];
+        Us[0] = fac;
+        for (int c = 0; c < 3; ++c) Us[1 + c] = fac * (c == dir ? SM : vK[K][c]);
+        Us[4] = fac * (EK[K] * rinvK[K] + (SM - nK[K]) * (SM + pK[K] / mK));
+        for (int c = 0; c < 5; ++c) F[c] = FK[K][c] + S * (Us[c] - UK[K][c]);
+    }
+    for (int s = 0; s < nspec; ++s)
+        F[5 + s] = F[0] * (F[0] >= 0.0 ? qL[5 + s] : qR[5 + s]);
+}
+
+/* ---- O2..O7 one RK stage of one box -------------------------------------- */
+/* Us: stage state of this box (ghosts filled), Ubase: U0 of this box (stage 1
+ * only), Uout: destination box (valid zones written). */
+static void advance_box(const oracle_params *p, const geom_t *g, int stage, double dt,
+                        const double *Us, const double *Ubase, double *Uout)
+{
+    const int ng = g->ng, nq = g->nq, nflux = g->nflux, nvar = g->nvar;
+    const size_t cs = g->comp_stride;
+    /* O2: primitives on every padded zone */
+    double *q = (double *)malloc(sizeof(double) * cs * nq);
+    double *Uc = (double *)malloc(sizeof(double) * nvar);
+    double *qz = (double *)malloc(sizeof(double) * nq);
+    for (size_t z = 0; z < cs; ++z) {
+        for (int c = 0; c < nvar; ++c) Uc[c] = Us[c * cs + z];
+        oracle_cons_to_prim(p->gamma, p->small_dens, p->small_pres, p->nspec, Uc, qz);
+        for (int c = 0; c < nq; ++c) q[c * cs + z] = qz[c];
+    }
+    /* O3-O5: face fluxes per direction.  F[d] holds NFLUX x (faces of d),
+     * face (i,j,k) of direction d = low face of valid zone (i,j,k), with the
+     * index along d running 0..nb[d]. */
+    double *F[3];
+    size_t fdim[3][3];
+    for (int d = 0; d < 3; ++d) {
+        for (int e = 0; e < 3; ++e) fdim[d][e] = g->nb[e] + (e == d ? 1 : 0);
+        F[d] = (double *)malloc(sizeof(double) * nflux * fdim[d][0] * fdim[d][1] * fdim[d][2]);
+    }
+    int nmax = 0;
+    for (int d = 0; d < 3; ++d) if (g->nt[d] > nmax) nmax = g->nt[d];
+    double *line = (double *)malloc(sizeof(double) * nmax * nq);
+    double *sl = (double *)malloc(sizeof(double) * nmax);
+    double *ed = (double *)malloc(sizeof(double) * nmax);
+    double *lL = (double *)malloc(sizeof(double) * nmax * nq);
+    double *lR = (double *)malloc(sizeof(double) * nmax * nq);
+    double *fL = (double *)malloc(sizeof(double) * nq);
+    double *fR = (double *)malloc(sizeof(double) * nq);
+    double *Ff = (double *)malloc(sizeof(double) * nflux);
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        const int n = g->nb[d] + 6; /* zones -3 .. nb+2 along d */
+        const size_t fcs = fdim[d][0] * fdim[d][1] * fdim[d][2];
+        for (int t2 = 0; t2 < g->nb[d2]; ++t2)
+        for (int t1 = 0; t1 < g->nb[d1]; ++t1) {
+            int ijk[3];
+            ijk[d1] = t1 + ng;
+            ijk[d2] = t2 + ng;
+            for (int c = 0; c < nq; ++c) {
+                for (int m = 0; m < n; ++m) {
+                    ijk[d] = m - 3 + ng;
+                    line[c * nmax + m] = q[c * cs + zidx(g, ijk[0], ijk[1], ijk[2])];
+                }
+                oracle_ppm_line(line + c * nmax, n, sl, ed, lL + c * nmax, lR + c * nmax);
+            }
+            /* face f (0..nb[d]) lies between line zones m = f+2 and m = f+3 */
+            for (int f = 0; f <= g->nb[d]; ++f) {
+                for (int c = 0; c < nq; ++c) {
+                    fL[c] = lR[c * nmax + f + 2];
+                    fR[c] = lL[c * nmax + f + 3];
+                }
+                oracle_hllc(d, p->gamma, p->small_dens, p->small_pres, p->nspec, fL, fR, Ff);
+                int fi[3];
+                fi[d] = f; fi[d1] = t1; fi[d2] = t2;
+                size_t fz = ((size_t)fi[2] * fdim[d][1] + fi[1]) * fdim[d][0] + fi[0];
+                for (int c = 0; c < nflux; ++c) F[d][c * fcs + fz] = Ff[c];
+            }
+        }
+    }
+    /* O6 + O7 */
+    const int has_grav = !(p->grav[0] == 0.0 && p->grav[1] == 0.0 && p->grav[2] == 0.0);
+    const double floor_rhoe = p->small_pres * (1.0 / (p->gamma - 1.0));
+    double *L = (double *)malloc(sizeof(double) * nflux);
+    for (int k = 0; k < g->nb[2]; ++k)
+    for (int j = 0; j < g->nb[1]; ++j)
+    for (int i = 0; i < g->nb[0]; ++i) {
+        size_t z = zidx(g, i + ng, j + ng, k + ng);
+        size_t fx0 = ((size_t)k * fdim[0][1] + j) * fdim[0][0] + i, fx1 = fx0 + 1;
+        size_t fy0 = ((size_t)k * fdim[1][1] + j) * fdim[1][0] + i, fy1 = fy0 + fdim[1][0];
+        size_t fz0 = ((size_t)k * fdim[2][1] + j) * fdim[2][0] + i, fz1 = fz0 + fdim[2][0] * fdim[2][1];
+        size_t fcx = fdim[0][0] * fdim[0][1] * fdim[0][2];
+        size_t fcy = fdim[1][0] * fdim[1][1] * fdim[1][2];
+        size_t fcz = fdim[2][0] * fdim[2][1] * fdim[2][2];
+        for (int c = 0; c < nflux; ++c) {
+            L[c] = -(F[0][c * fcx + fx1] - F[0][c * fcx + fx0]) * g->dxinv[0]
+                   - (F[1][c * fcy + fy1] - F[1][c * fcy + fy0]) * g->dxinv[1]
+                   - (F[2][c * fcz + fz1] - F[2][c * fcz + fz0]) * g->dxinv[2];
+        }
+        if (has_grav) {
+            double rho = Us[0 * cs + z], mx = Us[1 * cs + z], my = Us[2 * cs + z], mz = Us[3 * cs + z];
+            L[1] += rho * p->grav[0];
+            L[2] += rho * p->grav[1];
+            L[3] += rho * p->grav[2];
+            L[4] += mx * p->grav[0] + my * p->grav[1] + mz * p->grav[2];
+        }
+        for (int c = 0; c < nflux; ++c) {
+            int sc = c < 5 ? c : c + 1;
+            double unew;
+            if (stage == 0) unew = Us[sc * cs + z] + dt * L[c];
+            else unew = HALF * Ubase[sc * cs + z] + HALF * (Us[sc * cs + z] + dt * L[c]);
+            Uout[sc * cs + z] = unew;
+        }
+        {   /* rho*e re-synchronisation (O7, S2) */
+            double rho = Uout[0 * cs + z], mx = Uout[1 * cs + z], my = Uout[2 * cs + z],
+                   mz = Uout[3 * cs + z], rE = Uout[4 * cs + z];
+            double K = HALF * (mx * mx + my * my + mz * mz) / rho;
+            double re = rE - K;
+            if (re < floor_rhoe) re = floor_rhoe;
+            Uout[5 * cs + z] = re;
+        }
+    }
+    free(L);
+    free(Ff); free(fR); free(fL); free(lR); free(lL); free(ed); free(sl); free(line);
+    for (int d = 0; d < 3; ++d) free(F[d]);
+    free(qz); free(Uc); free(q);
+}
+
+/* stage 0: reads U0 (ghosts filled), writes valid zones of U1.
+ * stage 1: reads U1 (ghosts filled) and U0, overwrites valid zones of U0. */
+int oracle_advance_stage(const oracle_params *p, int stage, double dt, double *U0, double *U1)
+{
+    geom_t g;
+    if (make_geom(p, &g) || !U0 || !U1) return -1;
+    if (stage != 0 && stage != 1) return -1;
+    /* boxes are independent within a stage; the loop over boxes
+     * may run on several host threads without changing any bit of the result */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < g.nboxes; ++b) {
+        size_t off = (size_t)b * g.box_stride;
+        if (stage == 0) advance_box(p, &g, 0, dt, U0 + off, NULL, U1 + off);
+        else advance_box(p, &g, 1, dt, U1 + off, U0 + off, U0 + off);
+    }
+    return 0;
+}
+
+/* ---- O8 CFL timestep (S9, S10) ------------------------------------------- */
+int oracle_estimate_dt(const oracle_params *p, const double *U0, double *dt_out)
+{
+    geom_t g;
+    if (make_geom(p, &g) || !U0 || !dt_out) return -1;
+    const int ng = g.ng;
+    const size_t cs = g.comp_stride;
+    double tmax = 0.0;
+    int bad = 0;
+    for (int b = 0; b < g.nboxes; ++b) {
+        const double *Ub = U0 + (size_t)b * g.box_stride;
+        for (int k = 0; k < g.nb[2]; ++k)
+        for (int j = 0; j < g.nb[1]; ++j)
+        for (int i = 0; i < g.nb[0]; ++i) {
+            size_t z = zidx(&g, i + ng, j + ng, k + ng);
+            double rho = dmax(Ub[0 * cs + z], p->small_dens);
+            double rinv = 1.0 / rho;
+            double u = Ub[1 * cs + z] * rinv, v = Ub[2 * cs + z] * rinv, w = Ub[3 * cs + z] * rinv;
+            double pr = dmax((p->gamma - 1.0) * Ub[5 * cs + z], p->small_pres);
+            double c = sqrt(p->gamma * pr * rinv);
+            double t = (fabs(u) + c) * g.dxinv[0] + (fabs(v) + c) * g.dxinv[1] + (fabs(w) + c) * g.dxinv[2];
+            if (!(t == t) || isinf(t)) bad = 1;
+            if (t > tmax) tmax = t;
+        }
+    }
+    if (bad || !(tmax > 0.0)) return -4;
+    *dt_out = p->cfl / tmax;
+    return 0;
+}
+
+/* ---- O9 conservation totals (Neumaier-compensated sum) ------------------- */
+int oracle_conserved_totals(const oracle_params *p, const double *U, double *totals)
+{
+    geom_t g;
+    if (make_geom(p, &g) || !U || !totals) return -1;
+    const int ng = g.ng;
+    const size_t cs = g.comp_stride;
+    const double vol = g.dx[0] * g.dx[1] * g.dx[2];
+    for (int c = 0; c < g.nflux; ++c) {
+        int sc = c < 5 ? c : c + 1;
+        double sum = 0.0, comp = 0.0;
+        for (int b = 0; b < g.nboxes; ++b) {
+            const double *Ub = U + (size_t)b * g.box_stride + sc * cs;
+            for (int k = 0; k < g.nb[2]; ++k)
+            for (int j = 0; j < g.nb[1]; ++j)
+            for (int i = 0; i < g.nb[0]; ++i) {
+                double x = Ub[zidx(&g, i + ng, j + ng, k + ng)];
+                double t = sum + x;
+                if (fabs(sum) >= fabs(x)) comp += (sum - t) + x;
+                else comp += (x - t) + sum;
+                sum = t;
+            }
+        }
+        totals[c] = (sum + comp) * vol;
+    }
+    return 0;
+}
+
+/* ---- one RK2 step (S17): estimate_dt; fill(0); stage(0); fill(1); stage(1) */
+int oracle_step(const oracle_params *p, double *U0, double *U1, double *dt_out)
+{
+    double dt;
+    int rc = oracle_estimate_dt(p, U0, &dt);
+    if (rc) return rc;
+    if ((rc = oracle_fill_ghosts(p, U0))) return rc;
+    if ((rc = oracle_advance_stage(p, 0, dt, U0, U1))) return rc;
+    if ((rc = oracle_fill_ghosts(p, U1))) return rc;
+    if ((rc = oracle_advance_stage(p, 1, dt, U0, U1))) return rc;
+    if (dt_out) *dt_out = dt;
+    return 0;
+}
+
+/* Same as oracle_step but with dt supplied by the caller (used for sampled
+ * sub-block parity at full size, where dt comes from the whole domain). */
+int oracle_step_fixed_dt(const oracle_params *p, double *U0, double *U1, double dt)
+{
+    int rc;
+    if ((rc = oracle_fill_ghosts(p, U0))) return rc;
+    if ((rc = oracle_advance_stage(p, 0, dt, U0, U1))) return rc;
+    if ((rc = oracle_fill_ghosts(p, U1))) return rc;
+    if ((rc = oracle_advance_stage(p, 1, dt, U0, U1))) return rc;
+    return 0;
+}
+
+int oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
