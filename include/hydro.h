@@ -1,0 +1,131 @@
+/*
+ * hydro.h -- C ABI of libhydro_b200: one explicit compressible-hydro advance (unsplit
+ * method of lines: gamma-law EOS, PPM with the Colella-Woodward limiter, HLLC on every
+ * x/y/z face, flux divergence + constant gravity, SSP-RK2, intra-GPU ghost fill, CFL
+ * reduction) of a Castro-style state on a uniform-level MultiFab of boxes with ghost
+ * zones, on ONE NVIDIA B200 (sm_100a).
+ *
+ * Problem statement: PAPER.md:35 (sec. II: MultiFab = collection of Fabs, a Fab = a
+ * contiguous index box with several components, "a four-dimensional array"),
+ * PAPER.md:49-57 (sec. III: per-zone parallel hydro kernels, the slope/reconstruction
+ * stencil), PAPER.md:71,75 (no allocation inside the step loop; simulation data stay on
+ * the device), PAPER.md:83 (nearest-neighbour coupling only).  The paper prints no
+ * equations; the scheme is the one BASELINE.json:north_star names, written out step by
+ * step in DESIGN.md sec. 2 (O1..O9).
+ *
+ * Pointers: every pointer named *_dev is DEVICE memory owned by the caller for the whole
+ * lifetime of the handle; every pointer named *_host is HOST memory.  No torch types, no
+ * C++ types; plain pointers and sizes only.
+ *
+ * State layout a1: FP64, SoA, one padded 3-D array per (box, component),
+ * i fastest:
+ *     idx = (((b*NVAR + c)*NZt + k)*NYt + j)*NXt + i,   b = (bk*NBy + bj)*NBx + bi,
+ *     NXt = nbox[0] + 2*ng (etc.), valid zone (i,j,k) of a box at (i+ng, j+ng, k+ng).
+ * Components c: 0 rho, 1 rho*u, 2 rho*v, 3 rho*w, 4 rho*E, 5 rho*e, 6+k rho*X_k.
+ * NVAR = 6 + nspec stored components; NFLUX = 5 + nspec conserved components (all but
+ * rho*e, which is re-synchronised from rho*E after every stage).
+ *
+ * Errors: every int-returning call returns 0 on success or a negative HYDRO_E* code; no
+ * exception or abort crosses this boundary.  hydro_last_error() gives a message.
+ */
+#ifndef HYDRO_B200_H
+#define HYDRO_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HYDRO_OK       0
+#define HYDRO_EINVAL  -1  /* null pointer, nbox does not divide ndom, ng < 3, stage not 0/1,
+                             periodic flag on one side only, buffer not 16-byte aligned      */
+#define HYDRO_ENOMEM  -2  /* scratch_bytes too small (or device allocation failed in
+                             hydro_run_host)                                                 */
+#define HYDRO_ECUDA   -3  /* CUDA launch/runtime error; text via hydro_last_error            */
+#define HYDRO_ESTATE  -4  /* estimate_dt met a non-finite or non-positive max signal speed   */
+
+#define HYDRO_BC_PERIODIC 0
+#define HYDRO_BC_OUTFLOW  1
+#define HYDRO_BC_REFLECT  2
+
+typedef struct {
+    int32_t ndom[3];            /* zones in the domain (x,y,z)                               */
+    int32_t nbox[3];            /* zones per box; must divide ndom (regular tiling)          */
+    int32_t ng;                 /* ghost zones per side, >= 3 (the scheme reads 3)           */
+    int32_t nspec;              /* passive species, >= 0                                     */
+    int32_t bc_lo[3], bc_hi[3]; /* HYDRO_BC_*; periodic must be set on both sides of a dim   */
+    double  prob_lo[3], prob_hi[3]; /* physical domain; dx = (prob_hi-prob_lo)/ndom          */
+    double  gamma, cfl;
+    double  grav[3];            /* constant acceleration; {0,0,0} disables the source        */
+    double  small_dens, small_pres; /* floors (1e-12, 1e-14 in all workloads)                */
+} hydro_params;
+
+typedef struct hydro_ctx *hydro_handle;
+
+/* Size queries (host only, no CUDA call).  Return 0 for invalid params.
+ * hydro_state_bytes   = nboxes * NVAR * NXt*NYt*NZt * 8   (one state, layout a1)
+ * hydro_scratch_bytes = stage-increment accumulator (NFLUX per valid zone), one face
+ *                       mass-flux array, and the reduction workspace. */
+size_t hydro_state_bytes(const hydro_params *p);
+size_t hydro_scratch_bytes(const hydro_params *p);
+
+/* Create a handle.  U0_dev, U1_dev: two states of hydro_state_bytes each; scratch_dev:
+ * at least hydro_scratch_bytes; all 16-byte aligned, all caller-owned device memory that
+ * must outlive the handle.  cuda_stream: a cudaStream_t (NULL = legacy default stream);
+ * every kernel of this handle is enqueued on it.  The library allocates a few bytes of
+ * pinned host memory for scalar read-back here and nothing afterwards.
+ * The caller writes the initial state (all NVAR components of the valid zones; ghosts
+ * may hold anything) into U0 before the first step, with rho*e consistent with rho*E. */
+int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_dev,
+               size_t scratch_bytes, void *cuda_stream, hydro_handle *out);
+
+/* O1 ghost fill: fill every ghost zone (faces, edges, corners) of every box
+ * and component of state `which` (0: U0, 1: U1) from the valid zone that owns it:
+ * periodic wrap, outflow = nearest valid zone, reflect = mirror with the wall-normal
+ * momentum negated.  Asynchronous on the handle's stream. */
+int hydro_fill_ghosts(hydro_handle h, int which);
+
+/* O2..O7 one SSP-RK2 stage.  stage 0: reads U0 (ghosts must be filled), writes the valid
+ * zones of U1 = U0 + dt*L(U0).  stage 1: reads U1 (ghosts filled) and U0, overwrites the
+ * valid zones of U0 = 0.5*U0 + 0.5*(U1 + dt*L(U1)).  rho*e is re-synchronised in the
+ * written state.  Does NOT fill ghosts.  Asynchronous on the handle's stream. */
+int hydro_advance_stage(hydro_handle h, int stage, double dt);
+
+/* O8 CFL timestep: dt = cfl / max over valid zones of U0 of sum_d (|u_d| + c)/dx_d.
+ * Writes *dt_host; synchronises the stream.  HYDRO_ESTATE if the maximum is not a
+ * positive finite number. */
+int hydro_estimate_dt(hydro_handle h, double *dt_host);
+
+/* O9 totals: totals_host[f] = sum over valid zones of conserved component f times
+ * dx*dy*dz, f = 0..NFLUX-1 (rho, rho*u, rho*v, rho*w, rho*E, rho*X_k).  Deterministic
+ * (fixed reduction tree, compensated).  Synchronises the stream. */
+int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
+
+/* Convenience: n whole RK2 steps = n x { estimate_dt; fill(0); stage(0); fill(1);
+ * stage(1) } without host round trips (dt stays on the device).  dt_last_host (may be
+ * NULL) receives the last dt; when it is non-NULL the call synchronises. */
+int hydro_step(hydro_handle h, int nsteps, double *dt_last_host);
+
+/* Number of kernel launches this handle has enqueued so far (for bench accounting). */
+long long hydro_launch_count(hydro_handle h);
+
+int hydro_destroy(hydro_handle h);
+
+/* Message of the last error on this handle; with h == NULL, of the last failed
+ * hydro_init / hydro_run_host on this thread.  Never NULL. */
+const char *hydro_last_error(hydro_handle h);
+
+/* End-to-end entry for callers without device buffers: U_host (hydro_state_bytes, layout
+ * a1, valid zones filled) is copied to the device, advanced nsteps RK2 steps, and copied
+ * back in place; dt_host[0..nsteps-1] (may be NULL) receives the timesteps and
+ * totals_host[NFLUX] (may be NULL) the final conserved totals.  Allocates and frees its
+ * own device memory (outside the step loop).  Synchronous. */
+int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt_host,
+                   double *totals_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYDRO_B200_H */

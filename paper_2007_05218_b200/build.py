@@ -1,0 +1,47 @@
+"""Build step: compile csrc/hydro_api.cu into paper_2007_05218_b200/libhydro_b200.so.
+
+nvcc cross-compiles for sm_100a without a GPU.  `python -m paper_2007_05218_b200.build`
+or build().  HYDRO_FMAD=0 builds with -fmad=false (every operation rounded separately, as
+the scheme's definition is written); the default lets ptxas contract a*b+c into FMA.
+"""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libhydro_b200.so")
+SOURCES = ["hydro_api.cu"]
+HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_yz.cuh", "ghost_reduce.cuh"]
+
+
+def nvcc_cmd(fmad: bool, out: str = LIB, extra=()):
+    return ["nvcc", "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+            f"-fmad={'true' if fmad else 'false'}", "-shared", "-Xcompiler", "-fPIC",
+            "-o", out, *extra, *[os.path.join(CSRC, s) for s in SOURCES]]
+
+
+def build(force: bool = False, fmad=None, verbose: bool = False) -> str:
+    if fmad is None:
+        fmad = os.environ.get("HYDRO_FMAD", "1") != "0"
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [
+        os.path.join(os.path.dirname(HERE), "include", "hydro.h"), os.path.abspath(__file__)]
+    stamp = LIB + ".flags"
+    flags = "fmad=%d" % int(fmad)
+    fresh = (os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == flags
+             and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps))
+    if fresh and not force:
+        return LIB
+    cmd = nvcc_cmd(fmad, extra=["-Xptxas", "-v"] if verbose else [])
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if verbose:
+        sys.stderr.write(res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
+    with open(stamp, "w") as f:
+        f.write(flags)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force=True, verbose="-v" in sys.argv))

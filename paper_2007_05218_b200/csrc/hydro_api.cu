@@ -1,0 +1,396 @@
+// hydro_api.cu -- the C ABI of include/hydro.h: validation, scratch carving and kernel
+// launches.  All arithmetic of the path runs in the kernels included below; this file
+// only marshals.  sm_100a only; no CPU fallback.
+#include "../../include/hydro.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+
+#include "ghost_reduce.cuh"
+#include "hydro_device.cuh"
+#include "sweep_x.cuh"
+#include "sweep_yz.cuh"
+
+using namespace hydro;
+
+namespace {
+
+constexpr int RED_BLOCKS = 148 * 8;   // reduction grids: 8 CTAs of 256 threads per SM
+constexpr int NS_MAX = 7;             // species per thread in the y/z species kernels
+constexpr int BS = 128;               // threads per CTA of the marching kernels
+
+thread_local std::string g_init_error = "";
+
+struct Carve {
+    size_t lacc, frho, part, totals, red, dtslot, total;
+};
+
+}  // namespace
+
+struct hydro_ctx {
+    hydro_params p;
+    Geom g;
+    double *U[2];
+    char *scratch;
+    Carve cv;
+    cudaStream_t stream;
+    double *pinned;           // nflux + 2 doubles of pinned host memory
+    long long launches;
+    int seglen[3];
+    int ns_max;
+    std::string err;
+};
+
+namespace {
+
+bool make_geom(const hydro_params *p, Geom &g, std::string &why)
+{
+    if (!p) { why = "null params"; return false; }
+    if (p->ng < 3) { why = "ng must be >= 3"; return false; }
+    if (p->nspec < 0) { why = "nspec must be >= 0"; return false; }
+    if (!(p->gamma > 1.0)) { why = "gamma must be > 1"; return false; }
+    std::memset(&g, 0, sizeof(g));
+    g.ng = p->ng; g.nspec = p->nspec; g.nvar = 6 + p->nspec; g.nflux = 5 + p->nspec;
+    g.nboxes = 1;
+    double dx[3];
+    for (int d = 0; d < 3; ++d) {
+        if (p->ndom[d] <= 0 || p->nbox[d] <= 0 || p->ndom[d] % p->nbox[d] != 0) {
+            why = "nbox must be positive and divide ndom"; return false;
+        }
+        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 2 || p->bc_hi[d] < 0 || p->bc_hi[d] > 2) {
+            why = "bc must be 0, 1 or 2"; return false;
+        }
+        if ((p->bc_lo[d] == HYDRO_BC_PERIODIC) != (p->bc_hi[d] == HYDRO_BC_PERIODIC)) {
+            why = "periodic must be set on both sides of a dimension"; return false;
+        }
+        if ((p->bc_lo[d] == HYDRO_BC_REFLECT || p->bc_hi[d] == HYDRO_BC_REFLECT) && p->ng > p->ndom[d]) {
+            why = "ng must not exceed ndom across a reflecting boundary"; return false;
+        }
+        if (!(p->prob_hi[d] > p->prob_lo[d])) { why = "prob_hi must exceed prob_lo"; return false; }
+        g.nb[d] = p->nbox[d]; g.nt[d] = p->nbox[d] + 2 * p->ng; g.NB[d] = p->ndom[d] / p->nbox[d];
+        g.ndom[d] = p->ndom[d]; g.bc_lo[d] = p->bc_lo[d]; g.bc_hi[d] = p->bc_hi[d];
+        g.nboxes *= g.NB[d];
+        dx[d] = (p->prob_hi[d] - p->prob_lo[d]) / p->ndom[d];
+        g.dxinv[d] = 1.0 / dx[d];
+        g.grav[d] = p->grav[d];
+    }
+    if (g.nboxes > 65535) { why = "more than 65535 boxes"; return false; }
+    g.cstride = (long long)g.nt[0] * g.nt[1] * g.nt[2];
+    g.bstride = g.cstride * g.nvar;
+    g.lcstride = (long long)g.nb[0] * g.nb[1] * g.nb[2];
+    g.lbstride = g.lcstride * g.nflux;
+    g.fbstride = (long long)(g.nb[0] + 1) * (g.nb[1] + 1) * (g.nb[2] + 1);
+    g.gamma = p->gamma; g.gm1 = p->gamma - 1.0; g.gm1inv = 1.0 / (p->gamma - 1.0);
+    g.small_dens = p->small_dens; g.small_pres = p->small_pres;
+    g.floor_rhoe = p->small_pres * g.gm1inv;
+    g.cfl = p->cfl;
+    g.vol = dx[0] * dx[1] * dx[2];
+    g.has_grav = !(p->grav[0] == 0.0 && p->grav[1] == 0.0 && p->grav[2] == 0.0);
+    return true;
+}
+
+size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+Carve carve(const Geom &g)
+{
+    Carve c;
+    size_t off = 0;
+    c.lacc = off;   off += up256((size_t)g.lbstride * g.nboxes * 8);
+    c.frho = off;   off += up256((size_t)g.fbstride * g.nboxes * 8);
+    c.part = off;   off += up256((size_t)g.nflux * RED_BLOCKS * 2 * 8);
+    c.totals = off; off += up256((size_t)g.nflux * 8);
+    c.red = off;    off += 256;
+    c.dtslot = off; off += 256;
+    c.total = off;
+    return c;
+}
+
+int fail(hydro_handle h, int code, const std::string &msg)
+{
+    if (h) h->err = msg; else g_init_error = msg;
+    return code;
+}
+
+int check_launch(hydro_handle h, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    h->launches++;
+    if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return HYDRO_OK;
+}
+
+int pick_seglen(const Geom &g, int dir)
+{
+    const char *env = getenv("HYDRO_SEGLEN");
+    if (env && atoi(env) > 0) return atoi(env) < g.nb[dir] ? atoi(env) : g.nb[dir];
+    // enough pencils to fill 148 SMs several times over? then march the whole box
+    const int T = dir == 1 ? 2 : 1;
+    long long pencils = (long long)g.nb[0] * g.nb[T] * g.nboxes;
+    int nseg = 1;
+    while (pencils * nseg < 148LL * 1024 && g.nb[dir] / (nseg * 2) >= 16) nseg *= 2;
+    return (g.nb[dir] + nseg - 1) / nseg;
+}
+
+template <int DIR, bool FINAL, int STAGE>
+void launch_species(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
+{
+    switch (ns) {
+#define CASE(N) case N: k_sweep_species<DIR, FINAL, STAGE, N, BS><<<grid, BS, 0, h->stream>>>(h->g, a); break;
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7)
+#undef CASE
+        default: break;
+    }
+}
+
+template <int DIR, bool FINAL, int STAGE>
+int sweep_dir(hydro_handle h, SweepArgs a)
+{
+    const Geom &g = h->g;
+    constexpr int T = DIR == 1 ? 2 : 1;
+    a.seglen = h->seglen[DIR];
+    const int nseg = (g.nb[DIR] + a.seglen - 1) / a.seglen;
+    dim3 grid((g.nb[0] * g.nb[T] + BS - 1) / BS, nseg, g.nboxes);
+    k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
+    int rc = check_launch(h, "k_sweep_hydro");
+    if (rc) return rc;
+    if (g.nspec > 0) {
+        const int ngroups = (g.nspec + h->ns_max - 1) / h->ns_max;
+        const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
+        int s0 = 0;
+        for (int gr = 0; gr < ngroups; ++gr) {
+            const int ns = base + (gr < rem ? 1 : 0);
+            a.sbase = s0;
+            launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
+            if ((rc = check_launch(h, "k_sweep_species"))) return rc;
+            s0 += ns;
+        }
+    }
+    return HYDRO_OK;
+}
+
+int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev)
+{
+    const Geom &g = h->g;
+    SweepArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.Us = h->U[stage];
+    a.Ubase = h->U[0];
+    a.Uout = h->U[stage == 0 ? 1 : 0];
+    a.Lacc = (double *)(h->scratch + h->cv.lacc);
+    a.Frho = (double *)(h->scratch + h->cv.frho);
+    a.dt = dt;
+    a.dt_dev = dt_dev;
+    {   // x sweep: one warp per 26-zone chunk of a row
+        constexpr int WARPS = 4;
+        const long long nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
+        const long long nw = nchunk * g.nb[1] * g.nb[2] * g.nboxes;
+        const long long blocks = (nw + WARPS - 1) / WARPS;
+        if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
+        k_sweep_x<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc);
+        int rc = check_launch(h, "k_sweep_x");
+        if (rc) return rc;
+    }
+    int rc = sweep_dir<1, false, 0>(h, a);
+    if (rc) return rc;
+    if (stage == 0) return sweep_dir<2, true, 0>(h, a);
+    return sweep_dir<2, true, 1>(h, a);
+}
+
+int fill_ghosts_impl(hydro_handle h, int which)
+{
+    const Geom &g = h->g;
+    constexpr int WARPS = 4;
+    const long long nw = (long long)g.nt[1] * g.nt[2] * g.nvar * g.nboxes;
+    const long long blocks = (nw + WARPS - 1) / WARPS;
+    if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "ghost grid too large");
+    k_fill_ghosts<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, h->U[which]);
+    return check_launch(h, "k_fill_ghosts");
+}
+
+int launch_dt(hydro_handle h)
+{
+    const long long nzone = h->g.lcstride * h->g.nboxes;
+    long long blocks = (nzone + 255) / 256;
+    if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
+    k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[0],
+                                                           (unsigned long long *)(h->scratch + h->cv.red),
+                                                           (double *)(h->scratch + h->cv.dtslot));
+    return check_launch(h, "k_estimate_dt");
+}
+
+int read_dt(hydro_handle h, double *dt_host)
+{
+    cudaError_t e = cudaMemcpyAsync(h->pinned, h->scratch + h->cv.dtslot, 16, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("dt read-back: ") + cudaGetErrorString(e));
+    const double dt = h->pinned[0], tmax = h->pinned[1];
+    if (!(tmax > 0.0) || !std::isfinite(tmax) || !std::isfinite(dt))
+        return fail(h, HYDRO_ESTATE, "estimate_dt: max signal speed is not a positive finite number");
+    *dt_host = dt;
+    return HYDRO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t hydro_state_bytes(const hydro_params *p)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why)) return 0;
+    return (size_t)g.bstride * g.nboxes * 8;
+}
+
+size_t hydro_scratch_bytes(const hydro_params *p)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why)) return 0;
+    return carve(g).total;
+}
+
+int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_dev, size_t scratch_bytes,
+               void *cuda_stream, hydro_handle *out)
+{
+    Geom g; std::string why;
+    if (!out) return fail(nullptr, HYDRO_EINVAL, "null out handle");
+    *out = nullptr;
+    if (!make_geom(p, g, why)) return fail(nullptr, HYDRO_EINVAL, why);
+    if (!U0_dev || !U1_dev || !scratch_dev) return fail(nullptr, HYDRO_EINVAL, "null device buffer");
+    if (((uintptr_t)U0_dev | (uintptr_t)U1_dev | (uintptr_t)scratch_dev) & 15)
+        return fail(nullptr, HYDRO_EINVAL, "device buffers must be 16-byte aligned");
+    if (U0_dev == U1_dev) return fail(nullptr, HYDRO_EINVAL, "U0 and U1 must be distinct");
+    Carve cv = carve(g);
+    if (scratch_bytes < cv.total) return fail(nullptr, HYDRO_ENOMEM, "scratch_bytes too small");
+    hydro_ctx *h = new (std::nothrow) hydro_ctx();
+    if (!h) return fail(nullptr, HYDRO_ENOMEM, "host allocation failed");
+    h->p = *p; h->g = g; h->U[0] = (double *)U0_dev; h->U[1] = (double *)U1_dev;
+    h->scratch = (char *)scratch_dev; h->cv = cv; h->stream = (cudaStream_t)cuda_stream;
+    h->launches = 0; h->pinned = nullptr;
+    const char *env = getenv("HYDRO_NSMAX");
+    h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
+    for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
+    cudaError_t e = cudaMallocHost((void **)&h->pinned, (size_t)(g.nflux + 2) * 8);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 512, h->stream);
+    if (e != cudaSuccess) {
+        std::string msg = std::string("hydro_init: ") + cudaGetErrorString(e);
+        if (h->pinned) cudaFreeHost(h->pinned);
+        delete h;
+        return fail(nullptr, HYDRO_ECUDA, msg);
+    }
+    *out = h;
+    return HYDRO_OK;
+}
+
+int hydro_fill_ghosts(hydro_handle h, int which)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (which != 0 && which != 1) return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
+    return fill_ghosts_impl(h, which);
+}
+
+int hydro_advance_stage(hydro_handle h, int stage, double dt)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (stage != 0 && stage != 1) return fail(h, HYDRO_EINVAL, "stage must be 0 or 1");
+    return advance_stage_impl(h, stage, dt, nullptr);
+}
+
+int hydro_estimate_dt(hydro_handle h, double *dt_host)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (!dt_host) return fail(h, HYDRO_EINVAL, "null dt_host");
+    int rc = launch_dt(h);
+    if (rc) return rc;
+    return read_dt(h, dt_host);
+}
+
+int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (which != 0 && which != 1) return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
+    if (!totals_host) return fail(h, HYDRO_EINVAL, "null totals_host");
+    const Geom &g = h->g;
+    const long long nzone = g.lcstride * g.nboxes;
+    long long blocks = (nzone + 255) / 256;
+    if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
+    double *part = (double *)(h->scratch + h->cv.part);
+    double *tot = (double *)(h->scratch + h->cv.totals);
+    k_totals_partial<<<dim3((unsigned)blocks, g.nflux), 256, 0, h->stream>>>(g, h->U[which], part);
+    int rc = check_launch(h, "k_totals_partial");
+    if (rc) return rc;
+    k_totals_final<<<g.nflux, 32, 0, h->stream>>>(g, part, (int)blocks, tot);
+    if ((rc = check_launch(h, "k_totals_final"))) return rc;
+    cudaError_t e = cudaMemcpyAsync(h->pinned, tot, (size_t)g.nflux * 8, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("totals read-back: ") + cudaGetErrorString(e));
+    std::memcpy(totals_host, h->pinned, (size_t)g.nflux * 8);
+    return HYDRO_OK;
+}
+
+int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
+    const double *dt_dev = (const double *)(h->scratch + h->cv.dtslot);
+    int rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = launch_dt(h))) return rc;
+        if ((rc = fill_ghosts_impl(h, 0))) return rc;
+        if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev))) return rc;
+        if ((rc = fill_ghosts_impl(h, 1))) return rc;
+        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev))) return rc;
+    }
+    if (dt_last_host && nsteps > 0) return read_dt(h, dt_last_host);
+    return HYDRO_OK;
+}
+
+long long hydro_launch_count(hydro_handle h) { return h ? h->launches : 0; }
+
+int hydro_destroy(hydro_handle h)
+{
+    if (!h) return HYDRO_OK;
+    cudaStreamSynchronize(h->stream);
+    if (h->pinned) cudaFreeHost(h->pinned);
+    delete h;
+    return HYDRO_OK;
+}
+
+const char *hydro_last_error(hydro_handle h) { return h ? h->err.c_str() : g_init_error.c_str(); }
+
+int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt_host, double *totals_host)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why)) return fail(nullptr, HYDRO_EINVAL, why);
+    if (!U_host || nsteps < 0) return fail(nullptr, HYDRO_EINVAL, "null U_host or negative nsteps");
+    const size_t sb = (size_t)g.bstride * g.nboxes * 8, scb = carve(g).total;
+    void *U0 = nullptr, *U1 = nullptr, *sc = nullptr;
+    hydro_handle h = nullptr;
+    int rc = HYDRO_OK;
+    cudaError_t e = cudaMalloc(&U0, sb);
+    if (e == cudaSuccess) e = cudaMalloc(&U1, sb);
+    if (e == cudaSuccess) e = cudaMalloc(&sc, scb);
+    if (e != cudaSuccess) { rc = fail(nullptr, HYDRO_ENOMEM, std::string("hydro_run_host: ") + cudaGetErrorString(e)); goto done; }
+    e = cudaMemcpy(U0, U_host, sb, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { rc = fail(nullptr, HYDRO_ECUDA, std::string("H2D: ") + cudaGetErrorString(e)); goto done; }
+    if ((rc = hydro_init(p, U0, U1, sc, scb, nullptr, &h))) goto done;
+    for (int s = 0; s < nsteps && rc == HYDRO_OK; ++s) {
+        double dt = 0.0;
+        if (dt_host) { rc = hydro_step(h, 1, &dt); dt_host[s] = dt; }
+        else rc = hydro_step(h, 1, nullptr);
+    }
+    if (rc == HYDRO_OK && totals_host) rc = hydro_conserved_totals(h, 0, totals_host);
+    if (rc != HYDRO_OK) { g_init_error = h->err; goto done; }
+    e = cudaMemcpy(U_host, U0, sb, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) rc = fail(nullptr, HYDRO_ECUDA, std::string("D2H: ") + cudaGetErrorString(e));
+done:
+    if (h) hydro_destroy(h);
+    if (sc) cudaFree(sc);
+    if (U1) cudaFree(U1);
+    if (U0) cudaFree(U0);
+    return rc;
+}
+
+}  // extern "C"

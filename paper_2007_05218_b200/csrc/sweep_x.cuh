@@ -1,0 +1,88 @@
+// sweep_x.cuh -- x-direction reconstruct + Riemann + flux-difference kernel.
+//
+// x is the contiguous direction of layout a1, so a thread cannot own an x pencil without
+// strided (uncoalesced) access.  Instead a warp owns 32 consecutive zones of one row and the
+// PPM stencil is assembled with warp shuffles: each lane computes ITS zone's slope, edge
+// and monotonised parabola exactly once and hands them to its neighbours (de-duplicated,
+// unlike the one-thread-per-zone recompute of PAPER.md:51,57).  Lanes 3..28 produce zone
+// updates (26 per warp); the 3-lane aprons are the PPM halo.
+//
+// First sweep of a stage: WRITES the accumulator  Lacc_c = -(Fx_{i+1/2} - Fx_{i-1/2}) * dxinv.
+// Hydro variables and all species are handled here (species are transient per lane, so no
+// face mass-flux array is needed in x).
+#pragma once
+#include "hydro_device.cuh"
+
+namespace hydro {
+
+constexpr int XW_VALID = 26;   // zones updated per warp
+constexpr unsigned FULL = 0xffffffffu;
+
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(FULL, v, 1); }
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(FULL, v, 1); }
+
+// PPM along the lanes: returns the face states of face i+1/2 (between this lane's zone
+// and the next lane's): qLf = aR(i), qRf = aL(i+1).  Valid for lanes 2..28.
+__device__ __forceinline__ void ppm_lanes(double a, double& qLf, double& qRf)
+{
+    const double ap = shfl_dn1(a), am = shfl_up1(a);
+    const double s = ppm_slope(am, a, ap);             // lanes 1..30
+    const double sp = shfl_dn1(s);
+    const double e = ppm_edge(a, ap, s, sp);           // e_{i+1/2}, lanes 1..29
+    const double em = shfl_up1(e);                     // e_{i-1/2}, lanes 2..30
+    double aL, aR;
+    ppm_mono(em, e, a, aL, aR);                        // lanes 2..29
+    qLf = aR;
+    qRf = shfl_dn1(aL);                                // lanes 2..28
+}
+
+template <int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ Lacc)
+{
+    const int lane = threadIdx.x & 31;
+    const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
+    // warp -> (box, k, j, chunk), chunk fastest
+    long long w = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
+    const long long nw = (long long)nchunk * g.nb[1] * g.nb[2] * g.nboxes;
+    if (w >= nw) return;                               // whole warp leaves together
+    const int chunk = (int)(w % nchunk); w /= nchunk;
+    const int j = (int)(w % g.nb[1]); w /= g.nb[1];
+    const int k = (int)(w % g.nb[2]);
+    const int b = (int)(w / g.nb[2]);
+
+    const int i = chunk * XW_VALID + lane - 3;         // valid-zone index of this lane
+    int ip = i + g.ng;                                 // padded index
+    if (ip > g.nt[0] - 1) ip = g.nt[0] - 1;            // lanes past the halo: clamp (unused)
+    const long long row = ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0];
+    const double* Ub = U + (long long)b * g.bstride + row + ip;
+
+    double q[5], rinv;
+    cons_to_prim(g, ldg(Ub), ldg(Ub + g.cstride), ldg(Ub + 2 * g.cstride), ldg(Ub + 3 * g.cstride),
+                 ldg(Ub + 5 * g.cstride), q, rinv);
+    double qL[5], qR[5], F[5];
+#pragma unroll
+    for (int v = 0; v < 5; ++v) ppm_lanes(q[v], qL[v], qR[v]);
+    hllc<0>(g, qL, qR, F);                             // face i+1/2, lanes 2..28
+
+    const bool store = (lane >= 3) && (lane <= 2 + XW_VALID) && (i < g.nb[0]);
+    double* Lb = Lacc + (long long)b * g.lbstride + ((long long)k * g.nb[1] + j) * g.nb[0] + i;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+        const double Fm = shfl_up1(F[c]);
+        const double acc = -(F[c] - Fm) * g.dxinv[0];
+        if (store) Lb[c * g.lcstride] = acc;
+    }
+    const double Frho = F[0];
+    for (int s = 0; s < g.nspec; ++s) {
+        const double X = ldg(Ub + (6 + s) * g.cstride) * rinv;
+        double XL, XR;
+        ppm_lanes(X, XL, XR);
+        const double Fs = Frho * (Frho >= 0.0 ? XL : XR);
+        const double Fm = shfl_up1(Fs);
+        const double acc = -(Fs - Fm) * g.dxinv[0];
+        if (store) Lb[(5 + s) * g.lcstride] = acc;
+    }
+}
+
+}  // namespace hydro

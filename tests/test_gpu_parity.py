@@ -1,0 +1,188 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json north_star's: max relative error per
+component <= 1e-12 after one stage, <= 1e-10 after 10 steps, dt equal to 1e-14 relative
+(metric: SURVEY 8(c) S16); ghost fill (pure copies) bit-exact; totals to 1e-13 (S22)."""
+import numpy as np
+import pytest
+
+from oracle import oracle_binding as O
+from paper_2007_05218_b200 import workloads as W
+from parity_util import rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def hydro(wl):
+    from paper_2007_05218_b200.binding import Hydro
+    return Hydro(wl.params)
+
+
+# reduced instances of the five configs: several x-chunks (26-zone) with a ragged tail, pencil
+# counts that are not multiples of the CTA size, several boxes in every direction
+CASES = {
+    "cfg1_sod": lambda: W.config(1),
+    "cfg2_sedov_small": lambda: W.config(2, ndom=(48, 48, 48), nbox=(24, 24, 48)),
+    "cfg3_periodic_small": lambda: W.config(3, ndom=(80, 40, 60), nbox=(40, 20, 20)),
+    "cfg4_atmosphere_small": lambda: W.config(4, ndom=(32, 32, 64), nbox=(16, 32, 32)),
+    "cfg5_scaling_small": lambda: W.config(5, ndom=(64, 64, 64), nbox=(32, 32, 32)),
+    "cfg3_one_species_odd_box": lambda: W.config(3, ndom=(54, 30, 14), nbox=(27, 15, 7), nspec=1),
+}
+
+
+@pytest.mark.parametrize("bcs", [(0, 0, 0), (1, 1, 1), (2, 2, 2), (1, 0, 2), (2, 1, 0)])
+def test_ghost_fill_bit_exact(bcs):
+    wl = W.uniform((24, 12, 16), (12, 6, 8), 2, (1, 0, 0, 0, 1), bc=bcs)
+    rng = np.random.default_rng(1)
+    U = W.scatter_valid(wl, rng.standard_normal((wl.nvar, 16, 12, 24)), ghost_value=np.nan)
+    Uo = U.copy()
+    O.fill_ghosts(O.make_params(wl.params), Uo)
+    h = hydro(wl)
+    for which in (0, 1):
+        h.upload(U, which)
+        h.hydro_fill_ghosts(which)
+        assert np.array_equal(h.download(which).reshape(U.shape), Uo)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_one_stage_each_and_dt(name):
+    wl = CASES[name]()
+    U0 = W.initial_state(wl, ghost_value=np.nan)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    dt_o = O.estimate_dt(p, U0)
+    dt_g = h.hydro_estimate_dt()
+    assert abs(dt_g - dt_o) <= 1e-14 * dt_o
+    # stage 0
+    Uo0, Uo1 = U0.copy(), np.zeros_like(U0)
+    O.fill_ghosts(p, Uo0)
+    O.advance_stage(p, 0, dt_o, Uo0, Uo1)
+    h.hydro_fill_ghosts(0)
+    h.hydro_advance_stage(0, dt_o)
+    e0 = rel_err(wl, h.download(1).reshape(U0.shape), Uo1)
+    assert np.all(e0 <= 1e-12), e0
+    # stage 1 from the oracle's own U1 (isolates the stage)
+    O.fill_ghosts(p, Uo1)
+    h.upload(Uo1, 1)
+    O.advance_stage(p, 1, dt_o, Uo0, Uo1)
+    h.hydro_advance_stage(1, dt_o)
+    e1 = rel_err(wl, h.download(0).reshape(U0.shape), Uo0)
+    assert np.all(e1 <= 1e-12), e1
+
+
+@pytest.mark.parametrize("name,nsteps", [("cfg1_sod", 20), ("cfg2_sedov_small", 10), ("cfg3_periodic_small", 10),
+                                         ("cfg4_atmosphere_small", 10), ("cfg5_scaling_small", 5)])
+def test_multi_step(name, nsteps):
+    wl = CASES[name]()
+    U0 = W.initial_state(wl)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    for s in range(nsteps):
+        dt_o = O.step(p, Uo, Uo1)
+        dt_g = h.step_explicit()
+        assert abs(dt_g - dt_o) <= 1e-12 * dt_o, (s, dt_g, dt_o)       # state differs by rounding by now
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-10), e
+    tg, to = np.array(h.hydro_conserved_totals(0)), O.conserved_totals(p, Uo)
+    G = W.gather_valid(wl, np.abs(Uo))
+    scale = np.array([G[c if c < 5 else c + 1].sum() for c in range(wl.nflux)]) * np.prod(wl.dx)
+    assert np.all(np.abs(tg - to) <= 1e-10 * scale)
+
+
+def test_totals_match_oracle_on_same_state():
+    wl = CASES["cfg3_periodic_small"]()
+    U0 = W.initial_state(wl, ghost_value=1e30)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    tg, to = np.array(h.hydro_conserved_totals(0)), O.conserved_totals(O.make_params(wl.params), U0)
+    G = W.gather_valid(wl, np.abs(U0))
+    scale = np.array([G[c if c < 5 else c + 1].sum() for c in range(wl.nflux)]) * np.prod(wl.dx)
+    assert np.all(np.abs(tg - to) <= 1e-13 * scale)
+
+
+def test_fused_step_equals_explicit_calls_and_run_host():
+    from paper_2007_05218_b200 import binding as B
+    wl = CASES["cfg4_atmosphere_small"]()
+    U0 = W.initial_state(wl)
+    h1, h2 = hydro(wl), hydro(wl)
+    h1.upload(U0, 0); h2.upload(U0, 0)
+    dts = [h1.step_explicit() for _ in range(3)]
+    dt_last = h2.hydro_step(3)
+    assert dt_last == dts[-1]
+    A = h1.download(0)
+    assert np.array_equal(A, h2.download(0))
+    Uh = U0.copy()
+    dts_h, tot = B.hydro_run_host(B.make_params(wl.params), Uh, 3, want_totals=True)
+    assert dts_h == dts
+    va, vh = W.gather_valid(wl, A.reshape(U0.shape)), W.gather_valid(wl, Uh)
+    assert np.array_equal(va, vh)
+    assert tot == h1.hydro_conserved_totals(0)
+
+
+def test_decomposition_invariance_bitwise_on_gpu():
+    wl = W.config(3, ndom=(32, 32, 32), nbox=(32, 32, 32), nspec=2)
+    G0 = W.gather_valid(wl, W.initial_state(wl))
+    out = []
+    for nbox in [(32, 32, 32), (16, 16, 16), (8, 16, 32)]:
+        w = W.with_boxes(wl, nbox)
+        h = hydro(w)
+        h.upload(W.scatter_valid(w, G0, ghost_value=np.nan), 0)
+        h.hydro_step(2)
+        out.append(W.gather_valid(w, h.download(0).reshape(w.state_shape)))
+    assert np.array_equal(out[0], out[1]) and np.array_equal(out[0], out[2])
+
+
+def test_free_stream_and_floor_corner():
+    wl = W.uniform((32, 16, 16), (16, 16, 8), 2, (1.3, 0.7, -0.4, 0.25, 0.9), bc=W.OUTFLOW, X=(0.3, 0.7))
+    U0 = W.initial_state(wl)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    h.hydro_step(3)
+    G, R = W.gather_valid(wl, h.download(0).reshape(U0.shape)), W.gather_valid(wl, U0)
+    keep = [c for c in range(wl.nvar) if c != W.EINT]
+    assert np.array_equal(G[keep], R[keep])
+    # floors (parity unpinned corner: GPU vs oracle only): near-vacuum zone and negative rho*e
+    wl = W.config(3, ndom=(32, 16, 16), nbox=(16, 16, 16), nspec=1)
+    U0 = W.initial_state(wl).reshape(wl.state_shape)
+    U0[0, W.EINT, 8:12, 8:12, 8:12] = -1.0
+    U0[1, :, 9, 9, 9] *= 1e-14
+    U0 = U0.reshape(-1).reshape(wl.state_shape)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    dt_o = O.estimate_dt(p, Uo)
+    assert abs(h.hydro_estimate_dt() - dt_o) <= 1e-14 * dt_o
+    O.fill_ghosts(p, Uo); O.advance_stage(p, 0, dt_o, Uo, Uo1)
+    h.hydro_fill_ghosts(0); h.hydro_advance_stage(0, dt_o)
+    e = rel_err(wl, h.download(1).reshape(U0.shape), Uo1)
+    assert np.all(e <= 1e-12), e
+
+
+def test_error_codes():
+    from paper_2007_05218_b200 import binding as B
+    wl = W.uniform((16, 16, 16), (8, 8, 8), 0, (1, 0, 0, 0, 1))
+    h = hydro(wl)
+    assert B.lib().hydro_advance_stage(h.h, 2, 0.1) == B.HYDRO_EINVAL
+    assert B.lib().hydro_fill_ghosts(h.h, 5) == B.HYDRO_EINVAL
+    assert b"stage" in B.lib().hydro_last_error(h.h) or b"which" in B.lib().hydro_last_error(h.h)
+    U0 = W.initial_state(wl).reshape(wl.state_shape)
+    U0[3, W.MY, 6, 6, 6] = np.nan
+    h.upload(U0, 0)
+    with pytest.raises(B.HydroError) as ei:
+        h.hydro_estimate_dt()
+    assert ei.value.code == B.HYDRO_ESTATE
+    # too-small scratch and misaligned buffers
+    import ctypes as C
+    import torch
+    p = B.make_params(wl.params)
+    sb, scb = B.hydro_state_bytes(p), B.hydro_scratch_bytes(p)
+    a = torch.empty(sb // 8 + 2, dtype=torch.float64, device="cuda")
+    b = torch.empty(sb // 8 + 2, dtype=torch.float64, device="cuda")
+    s = torch.empty(scb, dtype=torch.uint8, device="cuda")
+    out = C.c_void_p()
+    assert B.lib().hydro_init(C.byref(p), a.data_ptr(), b.data_ptr(), s.data_ptr(), scb - 1, None, C.byref(out)) == B.HYDRO_ENOMEM
+    assert B.lib().hydro_init(C.byref(p), a.data_ptr() + 8, b.data_ptr(), s.data_ptr(), scb, None, C.byref(out)) == B.HYDRO_EINVAL
+    assert B.lib().hydro_init(C.byref(p), None, b.data_ptr(), s.data_ptr(), scb, None, C.byref(out)) == B.HYDRO_EINVAL
