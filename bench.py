@@ -1,0 +1,302 @@
+#!/usr/bin/env python
+"""bench.py -- zone-updates/s of the hydro hot path on BASELINE.json config 5 (512^3).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+
+A "step" is one whole pass of the hot path over the workload: one SSP-RK2 step =
+estimate_dt + 2 x (fill_ghosts + advance_stage) on every zone of the synthetic state.
+Prints ONE JSON line (rank 0).  See DESIGN.md sec. 7 for every field.
+
+  value      whole-job zone-updates/s with the state resident in HBM (CUDA events on the launch
+             stream, max over ranks).  N > 1 = N independent replicas (the
+             path named by north_star is single-GPU, "replicas only"), so scaling = "weak".
+  e2e        same metric through the C-ABI call that takes HOST buffers (hydro_run_host):
+             H2D of the state + step + D2H inside the timed region.
+  roofline   dominant kernel class: algorithmic bytes per launch / its mean launch duration
+             (CUDA event pairs recorded by the library around every launch of the timed region).
+  cpu_baseline  the CPU oracle, as it stands, timed on this box's host cores on a bounded
+             sample of the same recipe.
+--impl reference times only the oracle (there is no reference implementation to install).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2007_05218_b200 import workloads as W  # noqa: E402
+
+METRIC = "zone-updates/sec per RK2 step (FP64)"
+UNIT = "zone-updates/s"
+
+
+# ----------------------------------------------------------------------------- helpers
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes(wl, ns_groups):
+    """Algorithmic HBM bytes per launch of each kernel class: what the kernel
+    split must move -- every input once with the 3-zone PPM halo along the sweep direction, every
+    output once.  Returns {class: bytes per launch (mean over the launches of a step)}."""
+    nb, nvar, nflux, ns, ng = wl.nb, wl.nvar, wl.nflux, wl.nspec, wl.ng
+    Z = wl.zones
+    halo = [(nb[d] + 6) / nb[d] for d in range(3)]
+    face = [(nb[d] + 1) / nb[d] for d in range(3)]
+    nt = wl.nt
+    ghost_zones = wl.nboxes * (nt[0] * nt[1] * nt[2] - nb[0] * nb[1] * nb[2])
+    out = {}
+    out["fill_ghosts"] = 2 * nvar * 8 * ghost_zones
+    out["estimate_dt"] = 5 * 8 * Z
+    out["sweep_x"] = Z * ((nvar - 1) * 8 * halo[0] + nflux * 8)
+    out["hydro_y"] = Z * (5 * 8 * halo[1] + 2 * 5 * 8 + 8 * face[1])
+    # stage 0 / stage 1 mean for the z kernels (stage 1 also reads U0)
+    out["hydro_z"] = Z * (5 * 8 * halo[2] + 8 + 5 * 8 + 6 * 8 + 8 * face[2] + 0.5 * 5 * 8)
+    if ns:
+        g = np.mean(ns_groups)
+        out["species_y"] = Z * ((1 + g) * 8 * halo[1] + 8 * face[1] + 2 * g * 8)
+        out["species_z"] = Z * ((1 + g) * 8 * halo[2] + 8 * face[2] + 2 * g * 8 + 0.5 * g * 8)
+    return out
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                f = [x.strip() for x in out.stdout.strip().split(",")]
+                if len(f) >= 6:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[2 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm)}
+
+
+def oracle_sample(steps, warmup):
+    """The oracle, as it stands, on a bounded sample of the config-5 recipe: the 256^3 instance of the
+    same index-based generator (13 species, periodic, CFL 0.4) in 64^3 boxes."""
+    from oracle import oracle_binding as O
+    wl = W.config(5, ndom=(256, 256, 256), nbox=(64, 64, 64))
+    U0 = W.initial_state(wl, threads=8)
+    U1 = np.zeros_like(U0)
+    p = O.make_params(wl.params)
+    for _ in range(warmup):
+        O.step(p, U0, U1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        O.step(p, U0, U1)
+    el = time.perf_counter() - t0
+    return {"value": wl.zones * steps / el, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
+            "sample": f"config-5 recipe at 256^3 (13 species, 64 boxes of 64^3), {steps} RK2 steps, "
+                      f"OpenMP over boxes, {el:.1f} s"}, el / steps * 1e3, wl
+
+
+def workload_config(wl, n_cfg):
+    p = wl.params
+    return {"workload": f"BASELINE.json configs[{n_cfg - 1}] ({wl.name}): {'x'.join(map(str, p['ndom']))} zones in "
+                        f"{wl.nboxes} boxes of {'x'.join(map(str, p['nbox']))}, {wl.ng} ghost zones, "
+                        f"{wl.nspec} passive species (NVAR={wl.nvar}), gamma={p['gamma']:.6g}, cfl={p['cfl']}",
+            "zones": wl.zones, "state_gb": round(wl.state_bytes / 1e9, 3),
+            "l2_policy": "inputs_larger_than_l2 (every kernel streams >= 1 GB; no flush needed)"}
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 2))
+    cb, ms, wl = oracle_sample(steps, min(args.warmup, 1))
+    wl5 = W.config(args.config)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl5, args.config), "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "note": "no reference implementation exists (paper text only): this arm is the CPU oracle on a bounded "
+                    "sample of the workload"}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2007_05218_b200 import binding as B
+    from paper_2007_05218_b200 import build as build_mod
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the hydro path has no CPU fallback)")
+    build_mod.build()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    wl = W.config(args.config)
+    # ---- synthetic input, generated on the host, resident in pinned memory -------------
+    t0 = time.perf_counter()
+    pinned = True
+    try:
+        host = torch.empty(wl.state_shape, dtype=torch.float64, pin_memory=True)
+    except RuntimeError:
+        host, pinned = torch.empty(wl.state_shape, dtype=torch.float64), False
+    W.initial_state(wl, out=host.numpy(), threads=min(32, os.cpu_count() or 1))
+    t_gen = time.perf_counter() - t0
+
+    h = B.Hydro(wl.params, device=dev)
+    h.U0.copy_(host.reshape(-1), non_blocking=True)
+    torch.cuda.synchronize(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        h.hydro_step(1, want_dt=False)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = h.hydro_launch_count()
+    h.hydro_profile(1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(h.stream)
+    for _ in range(args.steps):
+        h.hydro_step(1, want_dt=False)
+    e1.record(h.stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    sampler.stop_flag = True
+    sampler.join(timeout=10)
+    prof = h.hydro_profile_read()
+    h.hydro_profile(0)
+    launches = h.hydro_launch_count() - launches0
+    dt_last = h.hydro_estimate_dt()
+    totals = h.hydro_conserved_totals(0)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * wl.zones * args.steps / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel class ------------------------------------------
+    peak, peak_src = measured_peaks()
+    ns_max = int(os.environ.get("HYDRO_NSMAX", "7"))
+    ngroups = max(1, -(-wl.nspec // ns_max)) if wl.nspec else 0
+    groups = [wl.nspec // ngroups + (1 if i < wl.nspec % ngroups else 0) for i in range(ngroups)] if ngroups else []
+    alg = algorithmic_bytes(wl, groups)
+    kernels = {}
+    tot_ms = sum(v[0] for v in prof.values())
+    for k, (ms, cnt) in prof.items():
+        if cnt and k in alg:
+            kernels[k] = {"ms_per_launch": ms / cnt, "launches_per_step": cnt / args.steps,
+                          "share_of_step": ms / tot_ms, "alg_gb_per_launch": alg[k] / 1e9,
+                          "gbs": alg[k] / 1e9 / (ms / cnt * 1e-3), "frac": alg[k] / 1e9 / (ms / cnt * 1e-3) / peak}
+    dom = max(kernels, key=lambda k: kernels[k]["share_of_step"])
+    step_alg = sum(alg[k] * kernels[k]["launches_per_step"] for k in kernels)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "whole_step": {"alg_bytes_per_zone_update": step_alg / wl.zones,
+                               "gbs": step_alg / 1e9 / (ms_step * 1e-3),
+                               "frac": step_alg / 1e9 / (ms_step * 1e-3) / peak,
+                               "frac_of_nominal_8000": step_alg / 1e9 / (ms_step * 1e-3) / 8000.0}}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")       # written from the committed ncu capture
+    if os.path.exists(tr):
+        try:
+            roofline["traffic"] = json.load(open(tr)).get(wl.name, {}).get(dom)
+        except Exception:
+            pass
+
+    # ---- e2e: host buffers through hydro_run_host ---------------------------------------
+    del h
+    torch.cuda.empty_cache()
+    e2e = None
+    if not args.no_e2e:
+        p = B.make_params(wl.params)
+        n_e2e = max(1, min(args.steps, 2))
+        B.hydro_run_host(p, host, 1)                            # warm-up (allocations, first touch)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            B.hydro_run_host(p, host, 1)
+        torch.cuda.synchronize(dev)
+        el = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([el], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            el = float(t.item())
+        e2e = {"value": world * wl.zones * n_e2e / el, "unit": UNIT, "h2d_bytes_per_step": wl.state_bytes,
+               "d2h_bytes_per_step": wl.state_bytes, "steps": n_e2e, "pinned_host": pinned,
+               "api": "hydro_run_host(params, U_host, 1 step)"}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu_baseline, _, _ = oracle_sample(1, 0)
+
+    if rank == 0:
+        cfg = workload_config(wl, args.config)
+        cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
+                    "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+                "zone_stages_per_s": 2 * value, "roofline": roofline, "kernels": kernels,
+                "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches),
+                "clocks": sampler.summary(), "dt_last": dt_last, "total_mass": totals[0]}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

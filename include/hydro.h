@@ -111,6 +111,16 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_last_host);
 /* Number of kernel launches this handle has enqueued so far (for bench accounting). */
 long long hydro_launch_count(hydro_handle h);
 
+/* Optional per-launch timing for measurement (bench.py's roofline object).  While enabled,
+ * every kernel launch of this handle is bracketed by a CUDA event pair on the handle's stream.
+ * hydro_profile_read synchronises, then writes the summed device time in ms and the launch
+ * count of each kernel class into ms_host[8] / count_host[8] and clears the record.
+ * Classes: 0 ghost fill, 1 dt reduction, 2 x sweep, 3 y hydro sweep, 4 y species sweep,
+ * 5 z hydro sweep + update, 6 z species sweep + update, 7 totals. */
+#define HYDRO_NCLASS 8
+int hydro_profile(hydro_handle h, int enable);
+int hydro_profile_read(hydro_handle h, double *ms_host, long long *count_host);
+
 int hydro_destroy(hydro_handle h);
 
 /* Message of the last error on this handle; with h == NULL, of the last failed

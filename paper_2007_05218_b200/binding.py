@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(HERE, "libhydro_b200.so")
 HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
-           "hydro_launch_count", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
+           "hydro_launch_count", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
 
 
 class HydroParams(C.Structure):
@@ -72,6 +72,8 @@ def lib():
     L.hydro_step.argtypes = [vp, C.c_int, dp]
     L.hydro_launch_count.restype = C.c_longlong
     L.hydro_launch_count.argtypes = [vp]
+    L.hydro_profile.argtypes = [vp, C.c_int]
+    L.hydro_profile_read.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
     L.hydro_destroy.argtypes = [vp]
     L.hydro_last_error.restype = C.c_char_p
     L.hydro_last_error.argtypes = [vp]
@@ -159,6 +161,18 @@ class Hydro:
 
     def hydro_launch_count(self):
         return lib().hydro_launch_count(self.h)
+
+    KERNEL_CLASSES = ["fill_ghosts", "estimate_dt", "sweep_x", "hydro_y", "species_y", "hydro_z", "species_z",
+                      "totals"]
+
+    def hydro_profile(self, enable):
+        self._check(lib().hydro_profile(self.h, int(enable)))
+
+    def hydro_profile_read(self):
+        ms = (C.c_double * 8)()
+        cnt = (C.c_longlong * 8)()
+        self._check(lib().hydro_profile_read(self.h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_CLASSES)}
 
     def step_explicit(self):
         """One RK2 step through the five separate calls (SURVEY 8(b) semantics)."""

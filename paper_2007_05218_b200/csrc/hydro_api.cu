@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "ghost_reduce.cuh"
 #include "hydro_device.cuh"
@@ -42,6 +43,11 @@ struct hydro_ctx {
     int seglen[3];
     int ns_max;
     std::string err;
+    // optional per-launch timing (hydro_profile): event pairs on the handle's stream
+    bool profiling;
+    struct Ev { cudaEvent_t a, b; int klass; };
+    std::vector<Ev> events;
+    cudaEvent_t pending;
 };
 
 namespace {
@@ -114,10 +120,27 @@ int fail(hydro_handle h, int code, const std::string &msg)
     return code;
 }
 
-int check_launch(hydro_handle h, const char *what)
+// kernel classes of hydro_profile_read
+enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIES_Z, K_TOTALS, K_NCLASS };
+
+void prof_begin(hydro_handle h)
+{
+    if (!h->profiling) return;
+    cudaEventCreate(&h->pending);
+    cudaEventRecord(h->pending, h->stream);
+}
+
+int check_launch(hydro_handle h, const char *what, int klass)
 {
     cudaError_t e = cudaGetLastError();
     h->launches++;
+    if (h->profiling && e == cudaSuccess) {
+        hydro_ctx::Ev ev;
+        ev.a = h->pending; ev.klass = klass;
+        cudaEventCreate(&ev.b);
+        cudaEventRecord(ev.b, h->stream);
+        h->events.push_back(ev);
+    }
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
     return HYDRO_OK;
 }
@@ -153,8 +176,9 @@ int sweep_dir(hydro_handle h, SweepArgs a)
     a.seglen = h->seglen[DIR];
     const int nseg = (g.nb[DIR] + a.seglen - 1) / a.seglen;
     dim3 grid((g.nb[0] * g.nb[T] + BS - 1) / BS, nseg, g.nboxes);
+    prof_begin(h);
     k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
-    int rc = check_launch(h, "k_sweep_hydro");
+    int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
     if (rc) return rc;
     if (g.nspec > 0) {
         const int ngroups = (g.nspec + h->ns_max - 1) / h->ns_max;
@@ -163,8 +187,9 @@ int sweep_dir(hydro_handle h, SweepArgs a)
         for (int gr = 0; gr < ngroups; ++gr) {
             const int ns = base + (gr < rem ? 1 : 0);
             a.sbase = s0;
+            prof_begin(h);
             launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
-            if ((rc = check_launch(h, "k_sweep_species"))) return rc;
+            if ((rc = check_launch(h, "k_sweep_species", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
             s0 += ns;
         }
     }
@@ -189,8 +214,9 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
         const long long nw = nchunk * g.nb[1] * g.nb[2] * g.nboxes;
         const long long blocks = (nw + WARPS - 1) / WARPS;
         if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
+        prof_begin(h);
         k_sweep_x<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc);
-        int rc = check_launch(h, "k_sweep_x");
+        int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }
     int rc = sweep_dir<1, false, 0>(h, a);
@@ -206,8 +232,9 @@ int fill_ghosts_impl(hydro_handle h, int which)
     const long long nw = (long long)g.nt[1] * g.nt[2] * g.nvar * g.nboxes;
     const long long blocks = (nw + WARPS - 1) / WARPS;
     if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "ghost grid too large");
+    prof_begin(h);
     k_fill_ghosts<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, h->U[which]);
-    return check_launch(h, "k_fill_ghosts");
+    return check_launch(h, "k_fill_ghosts", K_GHOST);
 }
 
 int launch_dt(hydro_handle h)
@@ -215,10 +242,11 @@ int launch_dt(hydro_handle h)
     const long long nzone = h->g.lcstride * h->g.nboxes;
     long long blocks = (nzone + 255) / 256;
     if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
+    prof_begin(h);
     k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[0],
                                                            (unsigned long long *)(h->scratch + h->cv.red),
                                                            (double *)(h->scratch + h->cv.dtslot));
-    return check_launch(h, "k_estimate_dt");
+    return check_launch(h, "k_estimate_dt", K_DT);
 }
 
 int read_dt(hydro_handle h, double *dt_host)
@@ -268,7 +296,7 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     if (!h) return fail(nullptr, HYDRO_ENOMEM, "host allocation failed");
     h->p = *p; h->g = g; h->U[0] = (double *)U0_dev; h->U[1] = (double *)U1_dev;
     h->scratch = (char *)scratch_dev; h->cv = cv; h->stream = (cudaStream_t)cuda_stream;
-    h->launches = 0; h->pinned = nullptr;
+    h->launches = 0; h->pinned = nullptr; h->profiling = false;
     const char *env = getenv("HYDRO_NSMAX");
     h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
@@ -318,11 +346,13 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
     if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
     double *part = (double *)(h->scratch + h->cv.part);
     double *tot = (double *)(h->scratch + h->cv.totals);
+    prof_begin(h);
     k_totals_partial<<<dim3((unsigned)blocks, g.nflux), 256, 0, h->stream>>>(g, h->U[which], part);
-    int rc = check_launch(h, "k_totals_partial");
+    int rc = check_launch(h, "k_totals_partial", K_TOTALS);
     if (rc) return rc;
+    prof_begin(h);
     k_totals_final<<<g.nflux, 32, 0, h->stream>>>(g, part, (int)blocks, tot);
-    if ((rc = check_launch(h, "k_totals_final"))) return rc;
+    if ((rc = check_launch(h, "k_totals_final", K_TOTALS))) return rc;
     cudaError_t e = cudaMemcpyAsync(h->pinned, tot, (size_t)g.nflux * 8, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("totals read-back: ") + cudaGetErrorString(e));
@@ -349,10 +379,34 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
 
 long long hydro_launch_count(hydro_handle h) { return h ? h->launches : 0; }
 
+int hydro_profile(hydro_handle h, int enable)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    h->profiling = enable != 0;
+    return HYDRO_OK;
+}
+
+int hydro_profile_read(hydro_handle h, double *ms_host, long long *count_host)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (!ms_host || !count_host) return fail(h, HYDRO_EINVAL, "null output");
+    for (int c = 0; c < K_NCLASS; ++c) { ms_host[c] = 0.0; count_host[c] = 0; }
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("profile_read: ") + cudaGetErrorString(e));
+    for (auto &ev : h->events) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, ev.a, ev.b) == cudaSuccess) { ms_host[ev.klass] += ms; count_host[ev.klass]++; }
+        cudaEventDestroy(ev.a); cudaEventDestroy(ev.b);
+    }
+    h->events.clear();
+    return HYDRO_OK;
+}
+
 int hydro_destroy(hydro_handle h)
 {
     if (!h) return HYDRO_OK;
     cudaStreamSynchronize(h->stream);
+    for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     if (h->pinned) cudaFreeHost(h->pinned);
     delete h;
     return HYDRO_OK;
