@@ -14,6 +14,7 @@
 #include "hydro_device.cuh"
 #include "sweep_x.cuh"
 #include "sweep_yz.cuh"
+#include "march_ring.cuh"
 
 using namespace hydro;
 
@@ -22,6 +23,7 @@ namespace {
 constexpr int RED_BLOCKS = 148 * 8;   // reduction grids: 8 CTAs of 256 threads per SM
 constexpr int NS_MAX = 7;             // species per thread in the y/z species kernels
 constexpr int BS = 128;               // threads per CTA of the marching kernels
+constexpr int RING_D = 8;             // depth of the TMA ring of the marching kernels
 
 thread_local std::string g_init_error = "";
 
@@ -42,6 +44,7 @@ struct hydro_ctx {
     long long launches;
     int seglen[3];
     int ns_max;
+    bool use_ring;            // TMA-ring marching kernels usable for this geometry
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs on the handle's stream
     bool profiling;
@@ -157,6 +160,27 @@ int pick_seglen(const Geom &g, int dir)
     return (g.nb[dir] + nseg - 1) / nseg;
 }
 
+template <typename K>
+void set_smem(K kernel, size_t bytes)
+{
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <int DIR, bool FINAL, int STAGE>
+void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
+{
+    switch (ns) {
+#define CASE(N) case N: { \
+        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + RING_D * 8; \
+        auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D>; \
+        static bool once = (set_smem(kern, sm), true); (void)once; \
+        kern<<<grid, BS, sm, h->stream>>>(h->g, a); } break;
+        CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7)
+#undef CASE
+        default: break;
+    }
+}
+
 template <int DIR, bool FINAL, int STAGE>
 void launch_species(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
 {
@@ -176,8 +200,20 @@ int sweep_dir(hydro_handle h, SweepArgs a)
     a.seglen = h->seglen[DIR];
     const int nseg = (g.nb[DIR] + a.seglen - 1) / a.seglen;
     dim3 grid((g.nb[0] * g.nb[T] + BS - 1) / BS, nseg, g.nboxes);
+    const bool ring = h->use_ring;
+    if (ring) {   // CTA = R row segments of W zones; rows may not fill the last CTA
+        const int W = g.nb[0] < BS ? g.nb[0] : BS, R = BS / W;
+        grid.x = (g.nb[T] * (g.nb[0] / W) + R - 1) / R;
+    }
     prof_begin(h);
-    k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
+    if (ring) {
+        constexpr int NROW = FINAL ? 6 : 5;
+        const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
+        auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D>;
+        static bool once = (set_smem(kern, sm), true); (void)once;
+        kern<<<grid, BS, sm, h->stream>>>(g, a);
+    } else
+        k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
     if (rc) return rc;
     if (g.nspec > 0) {
@@ -188,7 +224,8 @@ int sweep_dir(hydro_handle h, SweepArgs a)
             const int ns = base + (gr < rem ? 1 : 0);
             a.sbase = s0;
             prof_begin(h);
-            launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
+            if (ring) launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid);
+            else launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
             if ((rc = check_launch(h, "k_sweep_species", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
             s0 += ns;
         }
@@ -300,6 +337,12 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     const char *env = getenv("HYDRO_NSMAX");
     h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
+    {   // TMA bulk copies need 16-byte aligned row segments that tile the CTA exactly
+        const int W = g.nb[0] < BS ? g.nb[0] : BS;
+        const char *er = getenv("HYDRO_RING");
+        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) &&
+                      !(er && atoi(er) == 0);
+    }
     cudaError_t e = cudaMallocHost((void **)&h->pinned, (size_t)(g.nflux + 2) * 8);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 512, h->stream);
     if (e != cudaSuccess) {

@@ -26,6 +26,10 @@ CASES = {
     "cfg4_atmosphere_small": lambda: W.config(4, ndom=(32, 32, 64), nbox=(16, 32, 32)),
     "cfg5_scaling_small": lambda: W.config(5, ndom=(64, 64, 64), nbox=(32, 32, 32)),
     "cfg3_one_species_odd_box": lambda: W.config(3, ndom=(54, 30, 14), nbox=(27, 15, 7), nspec=1),
+    # TMA-ring marching kernels: two 64-zone row segments per CTA; ragged last CTA (6 rows of 4 per CTA)
+    "cfg2_sedov_wide_rows": lambda: W.config(2, ndom=(64, 32, 64), nbox=(64, 16, 32), nspec=2),
+    "cfg3_ragged_rows": lambda: W.config(3, ndom=(64, 12, 12), nbox=(32, 6, 6)),
+    "cfg5_256_wide_box": lambda: W.config(5, ndom=(256, 8, 8), nbox=(256, 8, 8), nspec=4),
 }
 
 
