@@ -19,40 +19,46 @@ __device__ __forceinline__ int map_global(const Geom& g, int d, int gi, bool& fl
     return gi < 0 ? -1 - gi : 2 * n - 1 - gi;
 }
 
-// One warp per padded row (j,k) of one (box, component).  Rows through the valid j,k range
-// only have their 2*ng end zones filled; rows in the ghost j/k range are filled whole.
-// Reads valid zones, writes ghost zones: disjoint, so one launch is race free.
-template <int WARPS>
-__global__ void __launch_bounds__(WARPS * 32)
+// One CTA per (padded k-plane, component, box); the plane's ghost zones are enumerated as a
+// flat task list so that consecutive threads touch consecutive zones.  A plane in the ghost
+// k-range is filled whole; a plane in the valid k-range has 2*ng whole ghost rows plus the
+// 2*ng end zones of each valid row.  The k mapping is done once per CTA.  Reads valid zones,
+// writes ghost zones: disjoint, so one launch is race free.
+__global__ void __launch_bounds__(256)
 k_fill_ghosts(const __grid_constant__ Geom g, double* __restrict__ U)
 {
-    const int lane = threadIdx.x & 31;
-    long long w = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    const long long rows = (long long)g.nt[1] * g.nt[2];
-    if (w >= rows * g.nvar * g.nboxes) return;
-    const int jl = (int)(w % g.nt[1]); w /= g.nt[1];
-    const int kl = (int)(w % g.nt[2]); w /= g.nt[2];
-    const int c = (int)(w % g.nvar);
-    const int b = (int)(w / g.nvar);
+    const int kl = blockIdx.x, c = blockIdx.y, b = blockIdx.z;
     const int bi = b % g.NB[0], bj = (b / g.NB[0]) % g.NB[1], bk = b / (g.NB[0] * g.NB[1]);
-
-    bool fy, fz;
-    const int gy = map_global(g, 1, bj * g.nb[1] + jl - g.ng, fy);
+    bool fz;
     const int gz = map_global(g, 2, bk * g.nb[2] + kl - g.ng, fz);
-    const int sbj = gy / g.nb[1], sbk = gz / g.nb[2];
-    const long long srow = ((long long)(gz - sbk * g.nb[2] + g.ng) * g.nt[1] + (gy - sbj * g.nb[1] + g.ng)) * g.nt[0];
-    double* dst = U + ((long long)b * g.nvar + c) * g.cstride + ((long long)kl * g.nt[1] + jl) * g.nt[0];
-    const bool interior = jl >= g.ng && jl < g.ng + g.nb[1] && kl >= g.ng && kl < g.ng + g.nb[2];
-    const int count = interior ? 2 * g.ng : g.nt[0];
-    for (int l = lane; l < count; l += 32) {
-        const int il = interior ? (l < g.ng ? l : g.nb[0] + l) : l;
-        bool fx;
+    const int sbk = gz / g.nb[2];
+    const int skl = gz - sbk * g.nb[2] + g.ng;
+    const bool kghost = kl < g.ng || kl >= g.ng + g.nb[2];
+    const int ng2 = 2 * g.ng;
+    const int nA = kghost ? g.nt[1] * g.nt[0] : ng2 * g.nt[0];      // whole rows
+    const int nB = kghost ? 0 : g.nb[1] * ng2;                        // row ends
+    double* dplane = U + ((long long)b * g.nvar + c) * g.cstride + (long long)kl * g.nt[1] * g.nt[0];
+    const double* splane = U + (long long)c * g.cstride + (long long)skl * g.nt[1] * g.nt[0];
+    for (int idx = threadIdx.x; idx < nA + nB; idx += blockDim.x) {
+        int jl, il;
+        if (idx < nA) {
+            const int row = idx / g.nt[0];
+            il = idx - row * g.nt[0];
+            jl = kghost ? row : (row < g.ng ? row : g.nb[1] + row);
+        } else {
+            const int r = idx - nA;
+            const int row = r / ng2, l = r - row * ng2;
+            jl = g.ng + row;
+            il = l < g.ng ? l : g.nb[0] + l;
+        }
+        bool fx, fy;
         const int gx = map_global(g, 0, bi * g.nb[0] + il - g.ng, fx);
-        const int sbi = gx / g.nb[0];
+        const int gy = map_global(g, 1, bj * g.nb[1] + jl - g.ng, fy);
+        const int sbi = gx / g.nb[0], sbj = gy / g.nb[1];
         const long long sb = ((long long)sbk * g.NB[1] + sbj) * g.NB[0] + sbi;
-        double v = U[(sb * g.nvar + c) * g.cstride + srow + (gx - sbi * g.nb[0] + g.ng)];
+        double v = splane[sb * g.bstride + (long long)(gy - sbj * g.nb[1] + g.ng) * g.nt[0] + (gx - sbi * g.nb[0] + g.ng)];
         if ((c == 1 && fx) || (c == 2 && fy) || (c == 3 && fz)) v = -v;
-        dst[il] = v;
+        dplane[(long long)jl * g.nt[0] + il] = v;
     }
 }
 

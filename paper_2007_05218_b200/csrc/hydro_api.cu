@@ -92,6 +92,7 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
     g.lcstride = (long long)g.nb[0] * g.nb[1] * g.nb[2];
     g.lbstride = g.lcstride * g.nflux;
     g.fbstride = (long long)(g.nb[0] + 1) * (g.nb[1] + 1) * (g.nb[2] + 1);
+    g.fbstride += g.fbstride & 1;                     // keep every box's face array 16-byte aligned
     g.gamma = p->gamma; g.gm1 = p->gamma - 1.0; g.gm1inv = 1.0 / (p->gamma - 1.0);
     g.small_dens = p->small_dens; g.small_pres = p->small_pres;
     g.floor_rhoe = p->small_pres * g.gm1inv;
@@ -265,12 +266,9 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
 int fill_ghosts_impl(hydro_handle h, int which)
 {
     const Geom &g = h->g;
-    constexpr int WARPS = 4;
-    const long long nw = (long long)g.nt[1] * g.nt[2] * g.nvar * g.nboxes;
-    const long long blocks = (nw + WARPS - 1) / WARPS;
-    if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "ghost grid too large");
+    if (g.nvar > 65535) return fail(h, HYDRO_EINVAL, "too many components for the ghost grid");
     prof_begin(h);
-    k_fill_ghosts<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, h->U[which]);
+    k_fill_ghosts<<<dim3(g.nt[2], g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
     return check_launch(h, "k_fill_ghosts", K_GHOST);
 }
 
