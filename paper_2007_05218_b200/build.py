@@ -17,8 +17,9 @@ HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_yz.cuh", "march_ring.cuh", 
 
 def nvcc_cmd(fmad: bool, out: str = LIB, extra=()):
     return ["nvcc", "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-            f"-fmad={'true' if fmad else 'false'}", "-shared", "-Xcompiler", "-fPIC",
-            "-o", out, *extra, *[os.path.join(CSRC, s) for s in SOURCES]]
+            f"-fmad={'true' if fmad else 'false'}", *([] if fmad else ["-DHYDRO_STRICT"]), "-shared", "-Xcompiler", "-fPIC",
+            "-o", out, *extra, *os.environ.get("HYDRO_NVCC_EXTRA", "").split(),
+            *[os.path.join(CSRC, s) for s in SOURCES]]
 
 
 def build(force: bool = False, fmad=None, verbose: bool = False) -> str:

@@ -172,7 +172,7 @@ void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
 {
     switch (ns) {
 #define CASE(N) case N: { \
-        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + RING_D * 8; \
+        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + 2 * RING_D * 8 + sizeof(RingDesc); \
         auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D>; \
         static bool once = (set_smem(kern, sm), true); (void)once; \
         kern<<<grid, BS, sm, h->stream>>>(h->g, a); } break;
@@ -209,7 +209,7 @@ int sweep_dir(hydro_handle h, SweepArgs a)
     prof_begin(h);
     if (ring) {
         constexpr int NROW = FINAL ? 6 : 5;
-        const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
+        const size_t sm = (size_t)RING_D * NROW * BS * 8 + 2 * RING_D * 8 + sizeof(RingDesc);
         auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D>;
         static bool once = (set_smem(kern, sm), true); (void)once;
         kern<<<grid, BS, sm, h->stream>>>(g, a);
@@ -338,7 +338,8 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     {   // TMA bulk copies need 16-byte aligned row segments that tile the CTA exactly
         const int W = g.nb[0] < BS ? g.nb[0] : BS;
         const char *er = getenv("HYDRO_RING");
-        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) &&
+        // and at most 64 copies per march step (2 descriptors per lane of warp 0): W >= 16
+        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && (W >= 16) &&
                       !(er && atoi(er) == 0);
     }
     cudaError_t e = cudaMallocHost((void **)&h->pinned, (size_t)(g.nflux + 2) * 8);

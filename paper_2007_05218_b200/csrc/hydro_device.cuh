@@ -59,21 +59,60 @@ __device__ __forceinline__ double ppm_edge(double a, double ap, double s, double
 // ---- O4: monotonised parabola edges of one zone (CW84 1.10) --------------------------
 __device__ __forceinline__ void ppm_mono(double el, double er, double a, double& aL, double& aR)
 {
-    double l = el, r = er;
-    if ((r - a) * (a - l) <= 0.0) {
-        l = a;
-        r = a;
-    } else {
-        const double d = r - l;
-        const double m = a - HALF * (l + r);
-        const double t = d * d * SIXTH;
-        const double dm = d * m;
-        if (dm > t) l = 3.0 * a - 2.0 * r;
-        else if (-t > dm) r = 3.0 * a - 2.0 * l;
-    }
-    aL = l;
-    aR = r;
+    // branch-free: every candidate is evaluated and the CW84 (1.10) cases pick among them, so
+    // the five variables of a zone stay in one basic block and interleave in the FP64 pipe.
+    // The selected values are the same expressions as in the if/else form of the definition.
+    const bool flat = (er - a) * (a - el) <= 0.0;
+    const double d = er - el;
+    const double m = a - HALF * (el + er);
+    const double t = d * d * SIXTH;
+    const double dm = d * m;
+    const bool over_l = dm > t;
+    const bool over_r = !over_l && (-t > dm);
+    const double l1 = over_l ? 3.0 * a - 2.0 * er : el;
+    const double r1 = over_r ? 3.0 * a - 2.0 * el : er;
+    aL = flat ? a : l1;
+    aR = flat ? a : r1;
 }
+
+// ---- division and square root ----------------------------------------------------------
+// HYDRO_STRICT (the -fmad=false build): IEEE-correct '/' and sqrt(), bit-for-bit the scheme's
+// definition.  Default build: branch-free Newton forms on the MUFU seeds (rcp/rsqrt.approx.f64),
+// faithful to <= 1 ulp for the normal-range operands of this path (densities >= small_dens,
+// pressures >= small_pres, wave-speed differences); no slow-path call, so no BSSY/BSYNC regions.
+#ifdef HYDRO_STRICT
+__device__ __forceinline__ double ddiv(double a, double b) { return a / b; }
+__device__ __forceinline__ double drcp(double b) { return 1.0 / b; }
+__device__ __forceinline__ double dsqrt(double x) { return sqrt(x); }
+#else
+__device__ __forceinline__ double drcp(double b)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+    double e = fma(-b, r, 1.0);      // seed is good to ~2^-20: two Newton steps reach 2^-80
+    r = fma(r, e, r);
+    e = fma(-b, r, 1.0);
+    return fma(r, e, r);
+}
+__device__ __forceinline__ double ddiv(double a, double b)
+{
+    const double r = drcp(b);
+    const double q = a * r;
+    return fma(fma(-b, q, a), r, q);
+}
+__device__ __forceinline__ double dsqrt(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double g = x * y, h = 0.5 * y;
+    double r = fma(-g, h, 0.5);      // coupled Newton on g ~ sqrt(x), h ~ 1/(2 sqrt(x))
+    g = fma(g, r, g); h = fma(h, r, h);
+    r = fma(-g, h, 0.5);
+    g = fma(g, r, g); h = fma(h, r, h);
+    g = fma(fma(-g, g, x), h, g);    // residual correction
+    return x > 0.0 ? g : 0.0;
+}
+#endif
 
 // ---- O5: HLLC flux of (rho, rho u, rho v, rho w, rho E) at one face ------------------
 // DIR = face normal.  qL/qR = (rho, u, v, w, p) left/right states.
@@ -84,23 +123,20 @@ __device__ __forceinline__ void hllc(const Geom& g, const double (&qL)[5], const
     const double rL = dmax(qL[0], g.small_dens), rR = dmax(qR[0], g.small_dens);
     const double pL = dmax(qL[4], g.small_pres), pR = dmax(qR[4], g.small_pres);
     const double nL = qL[1 + DIR], nR = qR[1 + DIR];
-    const double rinvL = 1.0 / rL, rinvR = 1.0 / rR;
-    const double cL = sqrt(g.gamma * pL * rinvL), cR = sqrt(g.gamma * pR * rinvR);
+    const double rinvL = drcp(rL), rinvR = drcp(rR);
+    const double cL = dsqrt(g.gamma * pL * rinvL), cR = dsqrt(g.gamma * pR * rinvR);
     const double SL = dmin(nL - cL, nR - cR);
     const double SR = dmax(nL + cL, nR + cR);
     const double EL = pL * g.gm1inv + HALF * rL * (qL[1] * qL[1] + qL[2] * qL[2] + qL[3] * qL[3]);
     const double ER = pR * g.gm1inv + HALF * rR * (qR[1] * qR[1] + qR[2] * qR[2] + qR[3] * qR[3]);
 
-    // which side supplies the flux, and whether a star state is needed
+    // Star-region quantities are always evaluated (branch-free); when the face is supersonic
+    // (SL >= 0 or SR <= 0) they are not selected.
     const bool star = !(SL >= 0.0) && !(SR <= 0.0);
-    double SM = 0.0, mL = 0.0, mR = 0.0;
-    bool left = (SL >= 0.0);
-    if (star) {
-        mL = rL * (SL - nL);
-        mR = rR * (SR - nR);
-        SM = (pR - pL + mL * nL - mR * nR) / (mL - mR);
-        left = (SM >= 0.0);
-    }
+    const double mL = rL * (SL - nL);
+    const double mR = rR * (SR - nR);
+    const double SM = ddiv(pR - pL + mL * nL - mR * nR, mL - mR);
+    const bool left = star ? (SM >= 0.0) : (SL >= 0.0);
     const double rK = left ? rL : rR, pK = left ? pL : pR, nK = left ? nL : nR;
     const double EK = left ? EL : ER;
     double vK[3];
@@ -119,22 +155,17 @@ __device__ __forceinline__ void hllc(const Geom& g, const double (&qL)[5], const
     FK[4] = (EK + pK) * nK;
     UK[0] = rK;
     UK[4] = EK;
-    if (star) {
-        const double rinvK = left ? rinvL : rinvR;
-        const double S = left ? SL : SR;
-        const double mK = left ? mL : mR;
-        const double fac = mK / (S - SM);
-        double Us[5];
-        Us[0] = fac;
+    const double rinvK = left ? rinvL : rinvR;
+    const double S = left ? SL : SR;
+    const double mK = left ? mL : mR;
+    const double fac = ddiv(mK, S - SM);
+    double Us[5];
+    Us[0] = fac;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) Us[1 + c] = fac * (c == DIR ? SM : vK[c]);
-        Us[4] = fac * (EK * rinvK + (SM - nK) * (SM + pK / mK));
+    for (int c = 0; c < 3; ++c) Us[1 + c] = fac * (c == DIR ? SM : vK[c]);
+    Us[4] = fac * (EK * rinvK + (SM - nK) * (SM + ddiv(pK, mK)));
 #pragma unroll
-        for (int c = 0; c < 5; ++c) F[c] = FK[c] + S * (Us[c] - UK[c]);
-    } else {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) F[c] = FK[c];
-    }
+    for (int c = 0; c < 5; ++c) F[c] = star ? FK[c] + S * (Us[c] - UK[c]) : FK[c];
 }
 
 // ---- O2: conserved -> primitive for the five hydro variables -------------------------
@@ -142,7 +173,7 @@ __device__ __forceinline__ void cons_to_prim(const Geom& g, double rho, double m
                                              double re, double (&q)[5], double& rinv)
 {
     const double r = dmax(rho, g.small_dens);
-    rinv = 1.0 / r;
+    rinv = drcp(r);
     q[0] = r;
     q[1] = mx * rinv;
     q[2] = my * rinv;

@@ -5,15 +5,35 @@
 // as R row segments of W contiguous zones.  For every march step one elected set of
 // threads issues cp.async.bulk (TMA, 1-D) copies of the step's rows -- W*8 contiguous
 // bytes per component per row segment -- into slot (step % D) of a D-deep ring, signalled
-// through an mbarrier with an expected-bytes count.  The copies run PD = D-KEEP steps
+// through a "full" mbarrier with an expected-bytes count.  The copies run D-KEEP-1 steps
 // ahead of the arithmetic, so the bytes in flight per SM are set by the ring depth and not
 // by how many registers a thread can spare: that is what the y/z sweeps lacked (ncu: 17 %
 // occupancy, fp64 pipe 19-30 %, DRAM 25-35 % of peak with plain per-thread loads).
+// Slot reuse is ordered by one __syncthreads per step (RING_CTASYNC=1, measured faster than
+// per-warp "empty" mbarriers, RING_CTASYNC=0).  The accumulator / face-flux / U0 rows that the
+// update needs are read with plain loads issued at the top of the step; pulling them into L2
+// ahead of time with cp.async.bulk.prefetch.L2 (RING_PF=1) measured slower and is off.
 // FINAL (z) kernels keep the last KEEP=3 slots alive so that the update of zone n-3 reads
 // its raw conserved state from shared memory instead of going back to L2.
 #pragma once
 #include "hydro_device.cuh"
 #include "sweep_yz.cuh"
+
+// tuning switches (overridable with -D for experiments)
+#ifndef RING_UNROLL
+#define RING_UNROLL 1      // unroll factor of the march loop
+#endif
+#ifndef RING_PF
+#define RING_PF 0          // cp.async.bulk.prefetch.L2 of the accumulator / face-flux / U0 rows
+#endif
+#ifndef RING_CTASYNC
+#define RING_CTASYNC 1     // 1: __syncthreads per step instead of per-warp slot release
+#endif
+#ifndef RING_MINB
+#define RING_MINB 3        // CTAs per SM the register allocation is capped for
+#endif
+#define RING_STR2(x) #x
+#define RING_STR(x) RING_STR2(x)
 
 namespace hydro {
 
@@ -39,6 +59,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
@@ -90,39 +118,38 @@ __device__ __forceinline__ long long zone_off(const Geom& g, int i, int t, int n
     return ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0] + (i + g.ng);
 }
 
-// Issue the copies of one march step: NROW component rows for each of the CTA's R row
-// segments.  comp(row) maps a ring row to a state component.  Called by all threads; thread
-// 0 arms the barrier, then the lanes of warp 0 issue the copies.
-template <int DIR, int BS, int NROW, typename CompOf>
-__device__ __forceinline__ void ring_issue(const Geom& g, const RingMap& m, const double* Ub, int cta, int n,
-                                           double* slot, uint64_t* bar, CompOf comp_of)
+// offset of valid zone (i, t, n) in the unpadded accumulator / face arrays of a DIR sweep;
+// ext = extent of the array along DIR (nb for the accumulator, nb+1 for the face array)
+template <int DIR>
+__device__ __forceinline__ long long flat_off(const Geom& g, int i, int t, int n, int ext)
 {
-    constexpr int T = (DIR == 1) ? 2 : 1;
-    const int ncopy = NROW * m.R;
-    if (threadIdx.x == 0) mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
-    if (threadIdx.x >= 32) return;                     // warp 0 issues, after its own expect_tx
-    for (int cpy = threadIdx.x; cpy < ncopy; cpy += 32) {
-        const int row = cpy / m.R, r = cpy - row * m.R;
-        const int xchunks = g.nb[0] / m.W;
-        const int rc = cta * m.R + r;
-        int t = rc / xchunks;
-        const int xc = rc - t * xchunks;
-        if (t >= g.nb[T]) t = g.nb[T] - 1;
-        const double* src = Ub + (long long)comp_of(row) * g.cstride + zone_off<DIR>(g, xc * m.W, t, n);
-        bulk_g2s(slot + row * BS + r * m.W, src, (uint32_t)(m.W * 8), bar);
-    }
+    return (DIR == 1) ? ((long long)t * ext + n) * g.nb[0] + i : ((long long)n * g.nb[1] + t) * g.nb[0] + i;
 }
+
+// Copy / prefetch descriptors held by the lanes of warp 0 (at most 2 each): pointer for
+// march step 0 and the destination offset inside a ring slot (copies), or the first step at
+// which the row exists (prefetches).  Per step a lane only adds step*stride.
+struct RingDesc {          // lives in shared memory: entry q*32 + lane
+    const double* src[64];
+    const double* pf[64];
+    long long pf_stride[64];
+    int dst[64];
+    int pf_first[64];
+};
 
 // ------------------------------------------------------------------------------------
 template <int DIR, bool FINAL, int STAGE, int BS, int D>
-__global__ void __launch_bounds__(BS)
+__global__ void __launch_bounds__(BS, RING_MINB)
 k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
 {
+    constexpr int T = (DIR == 1) ? 2 : 1;
     constexpr int NROW = FINAL ? 6 : 5;
     constexpr int KEEP = FINAL ? 3 : 0;
+    constexpr int NPF = 5 + ((FINAL && STAGE == 1) ? 5 : 0);        // Lacc rows (+ U0 rows)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
+    uint64_t* empty = full + D;
 
     const int tid = threadIdx.x;
     const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
@@ -131,23 +158,68 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
     const double* Ub = a.Us + (long long)b * g.bstride;
-    // ring row -> component: rho, mx, my, mz, rho*e, (rho*E)
-    auto comp_of = [](int row) { return row < 4 ? row : (row == 4 ? 5 : 4); };
+    const long long mstride = (DIR == 1) ? g.nt[0] : (long long)g.nt[0] * g.nt[1];
+    const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
+    double* Lbox = a.Lacc + (long long)b * g.lbstride;
+
+    RingDesc& ds = *reinterpret_cast<RingDesc*>(empty + D);
+    if (tid < 32) {
+        const int xchunks = g.nb[0] / m.W;
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const int cpy = tid + 32 * q;
+            ds.src[q * 32 + tid] = nullptr; ds.dst[q * 32 + tid] = 0; ds.pf[q * 32 + tid] = nullptr; ds.pf_first[q * 32 + tid] = 0; ds.pf_stride[q * 32 + tid] = 0;
+            const int row = cpy / m.R, r = cpy - row * m.R;
+            const int rc = blockIdx.x * m.R + r;
+            int t = rc / xchunks;
+            const int x0 = (rc - t * xchunks) * m.W;
+            if (t >= g.nb[T]) t = g.nb[T] - 1;
+            if (row < NROW) {
+                const int comp = row < 4 ? row : (row == 4 ? 5 : 4);   // rho, mx, my, mz, rho*e, (rho*E)
+                ds.src[q * 32 + tid] = Ub + (long long)comp * g.cstride + zone_off<DIR>(g, x0, t, m0 - 3);
+                ds.dst[q * 32 + tid] = row * BS + r * m.W;
+            }
+            if (row < NPF) {     // row of zone n-3 = m0-6+it: exists from step 6 on
+                ds.pf_first[q * 32 + tid] = 6;
+                if (row < 5) {
+                    ds.pf[q * 32 + tid] = Lbox + (long long)row * g.lcstride + flat_off<DIR>(g, x0, t, m0 - 6, g.nb[DIR]);
+                    ds.pf_stride[q * 32 + tid] = lmstride;
+                } else {
+                    ds.pf[q * 32 + tid] = a.Ubase + (long long)b * g.bstride + (long long)(row - 5) * g.cstride +
+                               zone_off<DIR>(g, x0, t, m0 - 6);
+                    ds.pf_stride[q * 32 + tid] = mstride;
+                }
+            }
+        }
+    }
+    auto issue = [&](int it) {      // warp 0 only
+        uint64_t* bar = &full[it % D];
+        double* slot = ring + (size_t)(it % D) * NROW * BS;
+        if (tid == 0) mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const double* src = ds.src[q * 32 + tid];
+            if (src) bulk_g2s(slot + ds.dst[q * 32 + tid], src + it * mstride, (uint32_t)(m.W * 8), bar);
+#if RING_PF
+            const double* pf = ds.pf[q * 32 + tid];
+            if (pf && it >= ds.pf_first[q * 32 + tid])
+                bulk_prefetch_l2(pf + it * ds.pf_stride[q * 32 + tid], (uint32_t)(m.W * 8));
+#endif
+        }
+    };
 
     if (tid == 0) {
-        for (int s = 0; s < D; ++s) mbar_init(&bars[s], 1);
+        for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BS / 32); }
         mbar_fence_init();
     }
     __syncthreads();
-    for (int it = 0; it < D - KEEP && it < nsteps; ++it)
-        ring_issue<DIR, BS, NROW>(g, m, Ub, blockIdx.x, m0 - 3 + it, ring + (size_t)(it % D) * NROW * BS,
-                                  &bars[it % D], comp_of);
+    if (tid < 32)
+        for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
-    const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
-    const long long l0 = (DIR == 1) ? (long long)m.t * g.nb[1] * g.nb[0] + m.i : (long long)m.t * g.nb[0] + m.i;
-    double* Lb = a.Lacc + (long long)b * g.lbstride + l0;
-    double* Fb = a.Frho + (long long)b * g.fbstride +
-                 ((DIR == 1) ? (long long)m.t * (g.nb[1] + 1) * g.nb[0] + m.i : (long long)m.t * g.nb[0] + m.i);
+    double* Lb = Lbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR]);
+    double* Fb = a.Frho + (long long)b * g.fbstride + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR] + 1);
+    const long long zo0 = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, 0);
     const double dinv = g.dxinv[DIR];
     const double dt = a.dt_dev ? *a.dt_dev : a.dt;
 
@@ -155,23 +227,23 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 #pragma unroll
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
 
+_Pragma(RING_STR(unroll RING_UNROLL))
     for (int it = 0; it < nsteps; ++it) {
         const int n = m0 - 3 + it;
         const int z = n - 3;
         const bool upd = (it >= 6);
-        // early, independent global loads for the update of zone z (consumed after the Riemann solve)
+        // early, independent global loads for the update of zone z (L2 hits: prefetched by warp 0)
         double lacc[5], ubase[5];
         if (upd) {
 #pragma unroll
             for (int c = 0; c < 5; ++c) lacc[c] = Lb[z * lmstride + c * g.lcstride];
             if (FINAL && STAGE == 1) {
-                const long long zo = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, z);
 #pragma unroll
-                for (int c = 0; c < 5; ++c) ubase[c] = a.Ubase[zo + c * g.cstride];
+                for (int c = 0; c < 5; ++c) ubase[c] = a.Ubase[zo0 + z * mstride + c * g.cstride];
             }
         }
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
-        mbar_wait(&bars[it % D], (uint32_t)((it / D) & 1));
+        mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         double q[5], rinv;
         cons_to_prim(g, slot[tid], slot[BS + tid], slot[2 * BS + tid], slot[3 * BS + tid], slot[4 * BS + tid], q, rinv);
         double qL[5], qR[5];
@@ -209,14 +281,14 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                         L[3] += us[0] * g.grav[2];
                         L[4] += us[1] * g.grav[0] + us[2] * g.grav[1] + us[3] * g.grav[2];
                     }
-                    const long long zo = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, z);
                     double un[5];
 #pragma unroll
                     for (int c = 0; c < 5; ++c) un[c] = rk_combine<STAGE>(us[c], (STAGE == 1) ? ubase[c] : 0.0, dt, L[c]);
-                    const double K = HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]) / un[0];
+                    const double K = ddiv(HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]), un[0]);
                     double re = un[4] - K;
                     if (re < g.floor_rhoe) re = g.floor_rhoe;
                     if (m.active) {
+                        const long long zo = zo0 + z * mstride;
 #pragma unroll
                         for (int c = 0; c < 5; ++c) a.Uout[zo + c * g.cstride] = un[c];
                         a.Uout[zo + 5 * g.cstride] = re;
@@ -226,24 +298,39 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 #pragma unroll
             for (int c = 0; c < 5; ++c) Fp[c] = F[c];
         }
-        __syncthreads();   // every thread is done with slot (it-KEEP)%D -> refill it
-        const int nx = it + D - KEEP;
-        if (nx < nsteps)
-            ring_issue<DIR, BS, NROW>(g, m, Ub, blockIdx.x, m0 - 3 + nx, ring + (size_t)(nx % D) * NROW * BS,
-                                      &bars[nx % D], comp_of);
+        // release slot (it-KEEP); warp 0 refills the slot released one step earlier
+#if RING_CTASYNC
+        __syncthreads();
+        if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
+#else
+        if (it >= KEEP) {
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
+        }
+        if (tid < 32) {
+            const int rel = it - KEEP - 1;
+            if (rel >= 0 && rel + D < nsteps) {
+                mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
+                issue(rel + D);
+            }
+        }
+#endif
     }
 }
 
 // ------------------------------------------------------------------------------------
 template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D>
-__global__ void __launch_bounds__(BS)
+__global__ void __launch_bounds__(BS, RING_MINB)
 k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
 {
+    constexpr int T = (DIR == 1) ? 2 : 1;
     constexpr int NROW = 1 + NS;
     constexpr int KEEP = FINAL ? 3 : 0;
+    constexpr int NPF = 1 + NS + ((FINAL && STAGE == 1) ? NS : 0);  // F_rho, Lacc rows (+ U0 rows)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
+    uint64_t* empty = full + D;
 
     const int tid = threadIdx.x;
     const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
@@ -251,24 +338,73 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     const int m0 = blockIdx.y * a.seglen;
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
-    const double* Ub = a.Us + (long long)b * g.bstride;
     const int sbase = a.sbase;
-    auto comp_of = [sbase](int row) { return row == 0 ? 0 : 5 + sbase + row; };   // rho, then rho*X_k
+    const double* Ub = a.Us + (long long)b * g.bstride;
+    const long long mstride = (DIR == 1) ? g.nt[0] : (long long)g.nt[0] * g.nt[1];
+    const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
+    double* Lbox = a.Lacc + (long long)b * g.lbstride + (long long)(5 + sbase) * g.lcstride;
+    const double* Fbox = a.Frho + (long long)b * g.fbstride;
+
+    RingDesc& ds = *reinterpret_cast<RingDesc*>(empty + D);
+    if (tid < 32) {
+        const int xchunks = g.nb[0] / m.W;
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const int cpy = tid + 32 * q;
+            ds.src[q * 32 + tid] = nullptr; ds.dst[q * 32 + tid] = 0; ds.pf[q * 32 + tid] = nullptr; ds.pf_first[q * 32 + tid] = 0; ds.pf_stride[q * 32 + tid] = 0;
+            const int row = cpy / m.R, r = cpy - row * m.R;
+            const int rc = blockIdx.x * m.R + r;
+            int t = rc / xchunks;
+            const int x0 = (rc - t * xchunks) * m.W;
+            if (t >= g.nb[T]) t = g.nb[T] - 1;
+            if (row < NROW) {
+                const int comp = row == 0 ? 0 : 5 + sbase + row;       // rho, then rho*X_k
+                ds.src[q * 32 + tid] = Ub + (long long)comp * g.cstride + zone_off<DIR>(g, x0, t, m0 - 3);
+                ds.dst[q * 32 + tid] = row * BS + r * m.W;
+            }
+            if (row < NPF) {
+                if (row == 0) {          // F_rho of face n-2 = m0-5+it: exists from step 5 on
+                    ds.pf[q * 32 + tid] = Fbox + flat_off<DIR>(g, x0, t, m0 - 5, g.nb[DIR] + 1);
+                    ds.pf_first[q * 32 + tid] = 5; ds.pf_stride[q * 32 + tid] = lmstride;
+                } else if (row <= NS) {  // Lacc of zone n-3
+                    ds.pf[q * 32 + tid] = Lbox + (long long)(row - 1) * g.lcstride + flat_off<DIR>(g, x0, t, m0 - 6, g.nb[DIR]);
+                    ds.pf_first[q * 32 + tid] = 6; ds.pf_stride[q * 32 + tid] = lmstride;
+                } else {                 // U0 rho*X_k of zone n-3
+                    ds.pf[q * 32 + tid] = a.Ubase + (long long)b * g.bstride + (long long)(6 + sbase + row - 1 - NS) * g.cstride +
+                               zone_off<DIR>(g, x0, t, m0 - 6);
+                    ds.pf_first[q * 32 + tid] = 6; ds.pf_stride[q * 32 + tid] = mstride;
+                }
+            }
+        }
+    }
+    auto issue = [&](int it) {      // warp 0 only
+        uint64_t* bar = &full[it % D];
+        double* slot = ring + (size_t)(it % D) * NROW * BS;
+        if (tid == 0) mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const double* src = ds.src[q * 32 + tid];
+            if (src) bulk_g2s(slot + ds.dst[q * 32 + tid], src + it * mstride, (uint32_t)(m.W * 8), bar);
+#if RING_PF
+            const double* pf = ds.pf[q * 32 + tid];
+            if (pf && it >= ds.pf_first[q * 32 + tid])
+                bulk_prefetch_l2(pf + it * ds.pf_stride[q * 32 + tid], (uint32_t)(m.W * 8));
+#endif
+        }
+    };
 
     if (tid == 0) {
-        for (int s = 0; s < D; ++s) mbar_init(&bars[s], 1);
+        for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BS / 32); }
         mbar_fence_init();
     }
     __syncthreads();
-    for (int it = 0; it < D - KEEP && it < nsteps; ++it)
-        ring_issue<DIR, BS, NROW>(g, m, Ub, blockIdx.x, m0 - 3 + it, ring + (size_t)(it % D) * NROW * BS,
-                                  &bars[it % D], comp_of);
+    if (tid < 32)
+        for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
-    const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
-    const long long l0 = (DIR == 1) ? (long long)m.t * g.nb[1] * g.nb[0] + m.i : (long long)m.t * g.nb[0] + m.i;
-    double* Lb = a.Lacc + (long long)b * g.lbstride + l0 + (long long)(5 + sbase) * g.lcstride;
-    const double* Fb = a.Frho + (long long)b * g.fbstride +
-                       ((DIR == 1) ? (long long)m.t * (g.nb[1] + 1) * g.nb[0] + m.i : (long long)m.t * g.nb[0] + m.i);
+    double* Lb = Lbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR]);
+    const double* Fb = Fbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR] + 1);
+    const long long zo0 = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, 0) + (long long)(6 + sbase) * g.cstride;
     const double dinv = g.dxinv[DIR];
     const double dt = a.dt_dev ? *a.dt_dev : a.dt;
 
@@ -276,6 +412,7 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
 #pragma unroll
     for (int v = 0; v < NS; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
 
+_Pragma(RING_STR(unroll RING_UNROLL))
     for (int it = 0; it < nsteps; ++it) {
         const int n = m0 - 3 + it;
         const int z = n - 3;
@@ -286,15 +423,13 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
 #pragma unroll
             for (int v = 0; v < NS; ++v) lacc[v] = Lb[z * lmstride + v * g.lcstride];
             if (FINAL && STAGE == 1) {
-                const long long zo = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, z) +
-                                     (long long)(6 + sbase) * g.cstride;
 #pragma unroll
-                for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo + v * g.cstride];
+                for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo0 + z * mstride + v * g.cstride];
             }
         }
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
-        mbar_wait(&bars[it % D], (uint32_t)((it / D) & 1));
-        const double rinv = 1.0 / dmax(slot[tid], g.small_dens);
+        mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
+        const double rinv = drcp(dmax(slot[tid], g.small_dens));
         const double* sz = ring + (size_t)((it + D - 3) % D) * NROW * BS;       // zone z's slot (FINAL)
 #pragma unroll
         for (int v = 0; v < NS; ++v) {
@@ -312,18 +447,27 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
                 } else {
                     const double us = sz[(1 + v) * BS + tid];
                     const double un = rk_combine<STAGE>(us, (STAGE == 1) ? ubase[v] : 0.0, dt, L);
-                    if (m.active)
-                        a.Uout[(long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, z) +
-                               (long long)(6 + sbase + v) * g.cstride] = un;
+                    if (m.active) a.Uout[zo0 + z * mstride + v * g.cstride] = un;
                 }
             }
             Fp[v] = Fs;
         }
+#if RING_CTASYNC
         __syncthreads();
-        const int nx = it + D - KEEP;
-        if (nx < nsteps)
-            ring_issue<DIR, BS, NROW>(g, m, Ub, blockIdx.x, m0 - 3 + nx, ring + (size_t)(nx % D) * NROW * BS,
-                                      &bars[nx % D], comp_of);
+        if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
+#else
+        if (it >= KEEP) {
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
+        }
+        if (tid < 32) {
+            const int rel = it - KEEP - 1;
+            if (rel >= 0 && rel + D < nsteps) {
+                mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
+                issue(rel + D);
+            }
+        }
+#endif
     }
 }
 

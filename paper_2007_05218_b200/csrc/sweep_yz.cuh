@@ -122,7 +122,7 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                     un[c] = rk_combine<STAGE>(us[c], ub, dt, L[c]);
                     a.Uout[zo + c * g.cstride] = un[c];
                 }
-                const double K = HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]) / un[0];
+                const double K = ddiv(HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]), un[0]);
                 double re = un[4] - K;
                 if (re < g.floor_rhoe) re = g.floor_rhoe;
                 a.Uout[zo + 5 * g.cstride] = re;
@@ -162,7 +162,7 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     for (int v = 0; v < NS; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
 
     for (int n = m0 - 3; n <= m1 + 2; ++n) {
-        const double rinv = 1.0 / dmax(ldg(Ub + n * mstride), g.small_dens);
+        const double rinv = drcp(dmax(ldg(Ub + n * mstride), g.small_dens));
         const bool haveF = (n >= m0 + 2);
         const double Frho = haveF ? ldg(Fb + (long long)(n - 2) * fmstride) : 0.0;
         const bool upd = (n >= m0 + 3);
