@@ -411,13 +411,17 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     double a1[NS], a2[NS], s1[NS], e1[NS], aR1[NS], Fp[NS];
 #pragma unroll
     for (int v = 0; v < NS; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
+    // F_rho of the face handled at step `it` is loaded one step ahead (ncu r01: 23-25 % of this
+    // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
+    double Fnext = 0.0;
 
 _Pragma(RING_STR(unroll RING_UNROLL))
     for (int it = 0; it < nsteps; ++it) {
         const int n = m0 - 3 + it;
         const int z = n - 3;
         const bool upd = (it >= 6);
-        const double Frho = (it >= 5) ? ldg(Fb + (long long)(n - 2) * lmstride) : 0.0;
+        const double Frho = Fnext;
+        if (it >= 4 && it + 1 < nsteps) Fnext = ldg(Fb + (long long)(n - 1) * lmstride);
         double lacc[NS], ubase[NS];
         if (upd) {
 #pragma unroll
@@ -431,6 +435,8 @@ _Pragma(RING_STR(unroll RING_UNROLL))
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         const double rinv = drcp(dmax(slot[tid], g.small_dens));
         const double* sz = ring + (size_t)((it + D - 3) % D) * NROW * BS;       // zone z's slot (FINAL)
+        // pass 1: reconstruction and face fluxes of all NS species (no global operand)
+        double dF[NS];
 #pragma unroll
         for (int v = 0; v < NS; ++v) {
             const double X = slot[(1 + v) * BS + tid] * rinv;
@@ -440,8 +446,14 @@ _Pragma(RING_STR(unroll RING_UNROLL))
             ppm_mono(e1[v], en, a2[v], aL, aR);
             const double Fs = Frho * (Frho >= 0.0 ? aR1[v] : aL);
             a2[v] = a1[v]; a1[v] = X; s1[v] = sn; e1[v] = en; aR1[v] = aR;
-            if (upd) {
-                const double L = lacc[v] - (Fs - Fp[v]) * dinv;
+            dF[v] = Fs - Fp[v];
+            Fp[v] = Fs;
+        }
+        // pass 2: accumulator / stage update (first use of this step's global loads)
+        if (upd) {
+#pragma unroll
+            for (int v = 0; v < NS; ++v) {
+                const double L = lacc[v] - dF[v] * dinv;
                 if (!FINAL) {
                     if (m.active) Lb[z * lmstride + v * g.lcstride] = L;
                 } else {
@@ -450,7 +462,6 @@ _Pragma(RING_STR(unroll RING_UNROLL))
                     if (m.active) a.Uout[zo0 + z * mstride + v * g.cstride] = un;
                 }
             }
-            Fp[v] = Fs;
         }
 #if RING_CTASYNC
         __syncthreads();
