@@ -212,7 +212,7 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- roofline of the dominant kernel class ------------------------------------------
     peak, peak_src = measured_peaks()
-    ns_max = int(os.environ.get("HYDRO_NSMAX", "7"))
+    ns_max = int(os.environ.get("HYDRO_NSMAX", "5"))
     ngroups = max(1, -(-wl.nspec // ns_max)) if wl.nspec else 0
     groups = [wl.nspec // ngroups + (1 if i < wl.nspec % ngroups else 0) for i in range(ngroups)] if ngroups else []
     alg = algorithmic_bytes(wl, groups)

@@ -30,7 +30,10 @@
 #define RING_CTASYNC 1     // 1: __syncthreads per step instead of per-warp slot release
 #endif
 #ifndef RING_MINB
-#define RING_MINB 3        // CTAs per SM the register allocation is capped for
+#define RING_MINB 3        // CTAs per SM the hydro kernels' register allocation is capped for
+#endif
+#ifndef RING_MINB_S
+#define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 #define RING_STR2(x) #x
 #define RING_STR(x) RING_STR2(x)
@@ -320,7 +323,7 @@ _Pragma(RING_STR(unroll RING_UNROLL))
 
 // ------------------------------------------------------------------------------------
 template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D>
-__global__ void __launch_bounds__(BS, RING_MINB)
+__global__ void __launch_bounds__(BS, RING_MINB_S)
 k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
 {
     constexpr int T = (DIR == 1) ? 2 : 1;

@@ -85,7 +85,17 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     double xc[XG];
 #pragma unroll
     for (int q = 0; q < XG; ++q) xc[q] = (q < g.nspec) ? ldg(Us + q * g.cstride) : 0.0;
-    for (int s0 = 0; s0 < g.nspec; s0 += XG) {
+    auto species = [&](double raw, int s) {
+        const double X = raw * rinv;
+        double XL, XR;
+        ppm_lanes(X, XL, XR);
+        const double Fs = Frho * (Frho >= 0.0 ? XL : XR);
+        const double Fm = shfl_up1(Fs);
+        const double acc = -(Fs - Fm) * g.dxinv[0];
+        if (store) Lb[(5 + s) * g.lcstride] = acc;
+    };
+    int s0 = 0;
+    for (; s0 + XG <= g.nspec; s0 += XG) {             // full groups: no per-species guard
         double xn[XG];
 #pragma unroll
         for (int q = 0; q < XG; ++q) {
@@ -93,21 +103,13 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
             xn[q] = (s < g.nspec) ? ldg(Us + s * g.cstride) : 0.0;
         }
 #pragma unroll
-        for (int q = 0; q < XG; ++q) {
-            const int s = s0 + q;
-            if (s < g.nspec) {                         // warp-uniform
-                const double X = xc[q] * rinv;
-                double XL, XR;
-                ppm_lanes(X, XL, XR);
-                const double Fs = Frho * (Frho >= 0.0 ? XL : XR);
-                const double Fm = shfl_up1(Fs);
-                const double acc = -(Fs - Fm) * g.dxinv[0];
-                if (store) Lb[(5 + s) * g.lcstride] = acc;
-            }
-        }
+        for (int q = 0; q < XG; ++q) species(xc[q], s0 + q);
 #pragma unroll
         for (int q = 0; q < XG; ++q) xc[q] = xn[q];
     }
+#pragma unroll
+    for (int q = 0; q < XG - 1; ++q)                   // tail group (warp-uniform guard)
+        if (s0 + q < g.nspec) species(xc[q], s0 + q);
 }
 
 }  // namespace hydro
