@@ -62,6 +62,112 @@ k_fill_ghosts(const __grid_constant__ Geom g, double* __restrict__ U)
     }
 }
 
+// ---- O1, split form used inside hydro_step ---------------------------------------------
+// The z (FINAL) sweeps write, next to every valid zone, the x-direction ghost images of that
+// zone (march_ring.cuh), so that every valid row (j, k valid) of the destination state is a
+// complete padded row.  What is left of the ghost fill are the ghost ROWS (j or k in the ghost
+// range): whole padded rows, each a copy of the complete padded row that the y/z mapping of O1
+// selects (same box column, so the x ends compose exactly as in k_fill_ghosts), with the sign
+// of rho*v / rho*w flipped across a reflecting y / z wall.  k_fill_ghost_rows does those copies
+// as 16-byte vectors.
+
+__device__ __forceinline__ int floor_div(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+// q-th ghost image (q = 0, 1, ...) along dimension d of valid zone l of box bd: the ghost zone
+// of box `dbox` at padded index `p` whose O1 source is this zone.  Returns false when there
+// are fewer than q+1 images.  Requires nb[d] >= ng.  Enumeration: the zone's own coordinate
+// (ghost of the adjacent boxes), then the coordinates the boundary condition maps onto it.
+__device__ __noinline__ bool dim_image(const Geom& g, int d, int bd, int l, int q, int& dbox, int& p, bool& flip)
+{
+    const int nb = g.nb[d], n = g.ndom[d], ng = g.ng, NB = g.NB[d];
+    const int g0 = bd * nb + l;
+    int cnt = 0;
+    // every box whose ghost range contains virtual coordinate v
+    auto visit = [&](int v, bool f) -> bool {
+        const int qb = floor_div(v, nb);
+        if (qb + 1 >= 0 && qb + 1 < NB && v >= (qb + 1) * nb - ng) {       // low ghosts of box qb+1
+            if (cnt == q) { dbox = qb + 1; p = v - (qb + 1) * nb + ng; flip = f; return true; }
+            ++cnt;
+        }
+        if (qb - 1 >= 0 && qb - 1 < NB && v < qb * nb + ng) {              // high ghosts of box qb-1
+            if (cnt == q) { dbox = qb - 1; p = v - (qb - 1) * nb + ng; flip = f; return true; }
+            ++cnt;
+        }
+        return false;
+    };
+    if (visit(g0, false)) return true;
+    if (g.bc_lo[d] == 0) {                     // periodic (both sides)
+        if (visit(g0 - n, false)) return true;
+        if (visit(g0 + n, false)) return true;
+        return false;
+    }
+    if (g.bc_lo[d] == 1 && g0 == 0) {
+        for (int v = -1; v >= -ng; --v) if (visit(v, false)) return true;
+    } else if (g.bc_lo[d] == 2 && g0 < ng) {
+        if (visit(-1 - g0, true)) return true;
+    }
+    if (g.bc_hi[d] == 1 && g0 == n - 1) {
+        for (int v = n; v < n + ng; ++v) if (visit(v, false)) return true;
+    } else if (g.bc_hi[d] == 2 && g0 >= n - ng) {
+        if (visit(2 * n - 1 - g0, true)) return true;
+    }
+    return false;
+}
+
+constexpr int GR_ROWS = 16;    // ghost rows per CTA of k_fill_ghost_rows
+
+// grid (ceil(nrows / GR_ROWS), nvar, nboxes), 256 threads.  nt[0] must be even (16-byte rows).
+__global__ void __launch_bounds__(256)
+k_fill_ghost_rows(const __grid_constant__ Geom g, double* __restrict__ U)
+{
+    __shared__ long long s_src[GR_ROWS], s_dst[GR_ROWS];
+    __shared__ double s_sgn[GR_ROWS];
+    const int c = blockIdx.y, b = blockIdx.z;
+    const int ng2 = 2 * g.ng;
+    const int nrows = g.nt[2] * g.nt[1] - g.nb[2] * g.nb[1];
+    const int r0 = blockIdx.x * GR_ROWS;
+    if (threadIdx.x < GR_ROWS) {
+        const int r = r0 + threadIdx.x;
+        long long src = -1, dst = 0;
+        double sgn = 1.0;
+        if (r < nrows) {
+            int kl, jl;
+            if (r < ng2 * g.nt[1]) {                                 // the 2*ng whole ghost planes
+                const int pz = r / g.nt[1];
+                kl = pz < g.ng ? pz : g.nb[2] + pz;
+                jl = r - pz * g.nt[1];
+            } else {                                                 // ghost rows of the valid planes
+                const int rr = r - ng2 * g.nt[1];
+                const int kz = rr / ng2, t = rr - kz * ng2;
+                kl = g.ng + kz;
+                jl = t < g.ng ? t : g.nb[1] + t;
+            }
+            const int bi = b % g.NB[0], bj = (b / g.NB[0]) % g.NB[1], bk = b / (g.NB[0] * g.NB[1]);
+            bool fy, fz;
+            const int gy = map_global(g, 1, bj * g.nb[1] + jl - g.ng, fy);
+            const int gz = map_global(g, 2, bk * g.nb[2] + kl - g.ng, fz);
+            const int sbj = gy / g.nb[1], sbk = gz / g.nb[2];
+            const long long sb = ((long long)sbk * g.NB[1] + sbj) * g.NB[0] + bi;
+            src = (sb * g.nvar + c) * g.cstride +
+                  ((long long)(gz - sbk * g.nb[2] + g.ng) * g.nt[1] + (gy - sbj * g.nb[1] + g.ng)) * g.nt[0];
+            dst = ((long long)b * g.nvar + c) * g.cstride + ((long long)kl * g.nt[1] + jl) * g.nt[0];
+            if ((c == 2 && fy) || (c == 3 && fz)) sgn = -1.0;
+        }
+        s_src[threadIdx.x] = src; s_dst[threadIdx.x] = dst; s_sgn[threadIdx.x] = sgn;
+    }
+    __syncthreads();
+    const int vpr = g.nt[0] >> 1;                                    // double2 per row
+    for (int e = threadIdx.x; e < GR_ROWS * vpr; e += blockDim.x) {
+        const int r = e / vpr, col = e - r * vpr;
+        const long long src = s_src[r];
+        if (src < 0) continue;
+        double2 v = __ldg(reinterpret_cast<const double2*>(U + src) + col);
+        const double sg = s_sgn[r];
+        v.x *= sg; v.y *= sg;
+        reinterpret_cast<double2*>(U + s_dst[r])[col] = v;
+    }
+}
+
 // ---- O8 ----------------------------------------------------------------------------
 // red[0] = running max of t (as ordered bits), red[1] = blocks-done counter,
 // dtslot[0] = dt, dtslot[1] = max t of the last reduction.

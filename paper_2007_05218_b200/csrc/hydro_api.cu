@@ -24,7 +24,10 @@ constexpr int RED_BLOCKS = 148 * 8;   // reduction grids: 8 CTAs of 256 threads 
 constexpr int NS_MAX = 5;             // species per thread in the y/z species kernels: 5 keeps the marching
                                       // kernels at 128 registers = 4 CTAs per SM (measured faster than 7 at 168 / 3)
 constexpr int BS = 128;               // threads per CTA of the marching kernels
-constexpr int RING_D = 8;             // depth of the TMA ring of the marching kernels
+#ifndef HYDRO_RING_D
+#define HYDRO_RING_D 8
+#endif
+constexpr int RING_D = HYDRO_RING_D;  // depth of the TMA ring of the marching kernels
 
 thread_local std::string g_init_error = "";
 
@@ -46,6 +49,7 @@ struct hydro_ctx {
     int seglen[3];
     int ns_max;
     bool use_ring;            // TMA-ring marching kernels usable for this geometry
+    bool split_ghosts;        // hydro_step: x ghost images written by the z sweeps + ghost-row copies
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs on the handle's stream
     bool profiling;
@@ -235,7 +239,7 @@ int sweep_dir(hydro_handle h, SweepArgs a)
     return HYDRO_OK;
 }
 
-int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev)
+int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev, bool xends = false)
 {
     const Geom &g = h->g;
     SweepArgs a;
@@ -247,6 +251,7 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     a.Frho = (double *)(h->scratch + h->cv.frho);
     a.dt = dt;
     a.dt_dev = dt_dev;
+    a.xends = (xends && h->use_ring) ? 1 : 0;
     {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const long long nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
@@ -271,6 +276,16 @@ int fill_ghosts_impl(hydro_handle h, int which)
     prof_begin(h);
     k_fill_ghosts<<<dim3(g.nt[2], g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
     return check_launch(h, "k_fill_ghosts", K_GHOST);
+}
+
+// ghost rows of state `which` (the part of O1 left when the z sweeps wrote the x images)
+int fill_ghost_rows_impl(hydro_handle h, int which)
+{
+    const Geom &g = h->g;
+    const int nrows = g.nt[2] * g.nt[1] - g.nb[2] * g.nb[1];
+    prof_begin(h);
+    k_fill_ghost_rows<<<dim3((nrows + GR_ROWS - 1) / GR_ROWS, g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
+    return check_launch(h, "k_fill_ghost_rows", K_GHOST);
 }
 
 int launch_dt(hydro_handle h)
@@ -343,6 +358,11 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
         h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && (W >= 16) &&
                       !(er && atoi(er) == 0);
     }
+    {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
+        const char *ef = getenv("HYDRO_SPLIT_GHOSTS");
+        h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng &&
+                          g.nb[2] >= g.ng && !(ef && atoi(ef) == 0);
+    }
     cudaError_t e = cudaMallocHost((void **)&h->pinned, (size_t)(g.nflux + 2) * 8);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 512, h->stream);
     if (e != cudaSuccess) {
@@ -409,12 +429,15 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
     if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
     const double *dt_dev = (const double *)(h->scratch + h->cv.dtslot);
     int rc;
+    const bool split = h->split_ghosts;
     for (int s = 0; s < nsteps; ++s) {
         if ((rc = launch_dt(h))) return rc;
-        if ((rc = fill_ghosts_impl(h, 0))) return rc;
-        if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev))) return rc;
-        if ((rc = fill_ghosts_impl(h, 1))) return rc;
-        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev))) return rc;
+        // the caller's U0 gets the full fill; after that stage 1 has left every valid row of U0
+        // complete (x images written by the z sweeps) and only the ghost rows remain
+        if ((rc = (split && s > 0) ? fill_ghost_rows_impl(h, 0) : fill_ghosts_impl(h, 0))) return rc;
+        if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev, split))) return rc;
+        if ((rc = split ? fill_ghost_rows_impl(h, 1) : fill_ghosts_impl(h, 1))) return rc;
+        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split))) return rc;
     }
     if (dt_last_host && nsteps > 0) return read_dt(h, dt_last_host);
     return HYDRO_OK;

@@ -18,6 +18,7 @@
 #pragma once
 #include "hydro_device.cuh"
 #include "sweep_yz.cuh"
+#include "ghost_reduce.cuh"
 
 // tuning switches (overridable with -D for experiments)
 #ifndef RING_UNROLL
@@ -85,6 +86,21 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         : "memory");
 }
 
+// non-blocking phase test by lane 0, broadcast to the warp
+__device__ __forceinline__ bool mbar_test_warp(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok = 0;
+    if ((threadIdx.x & 31) == 0) {
+        asm volatile(
+            "{\n"
+            ".reg .pred P1;\n"
+            "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, P1;\n"
+            "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    }
+    return __shfl_sync(0xffffffffu, ok, 0) != 0;
+}
+
 // Decomposition of a CTA into R row segments of W zones.
 struct RingMap {
     int W, R;        // zones per row segment, row segments per CTA
@@ -127,6 +143,44 @@ template <int DIR>
 __device__ __forceinline__ long long flat_off(const Geom& g, int i, int t, int n, int ext)
 {
     return (DIR == 1) ? ((long long)t * ext + n) * g.nb[0] + i : ((long long)n * g.nb[1] + t) * g.nb[0] + i;
+}
+
+
+// x-direction ghost images of this thread's pencil (FINAL kernels with a.xends).  With boxes
+// at least ng wide a zone has at most two groups of images, one per side; a group is a single
+// ghost zone (box interface, periodic wrap, reflecting wall) or the run of ng consecutive ghost
+// zones an outflow wall copies from its edge zone.  Group q: first image at offset d[q] from the
+// zone, n[q] images, consecutive ones `step[q]` doubles apart, f[q] = reflected.
+struct XEnds {
+    long long d[2];
+    int n[2], step[2];
+    bool f[2];
+    bool any;        // the zone has images
+    bool single;     // exactly one image (group 0): the common case, unrolled in the kernels
+};
+__device__ __forceinline__ XEnds xends_setup(const Geom& g, bool on, int b, int i)
+{
+    XEnds x;
+    x.d[0] = x.d[1] = 0; x.n[0] = x.n[1] = 0; x.step[0] = x.step[1] = 1; x.f[0] = x.f[1] = false;
+    if (on) {
+        const int bi = b % g.NB[0];
+        int db, p, q = 0, grp = -1, ldb = 0, lp = 0;
+        bool f;
+        while (dim_image(g, 0, bi, i, q, db, p, f)) {
+            const bool run = grp >= 0 && db == ldb && f == x.f[grp] && (p == lp + 1 || p == lp - 1) &&
+                             (x.n[grp] == 1 || p - lp == x.step[grp]);
+            if (run) { x.step[grp] = p - lp; ++x.n[grp]; }
+            else if (grp < 1) {
+                ++grp;
+                x.d[grp] = (long long)(db - bi) * g.bstride + (p - (i + g.ng));
+                x.n[grp] = 1; x.f[grp] = f;
+            }
+            ldb = db; lp = p; ++q;
+        }
+    }
+    x.any = (x.n[0] | x.n[1]) != 0;
+    x.single = x.n[0] == 1 && x.n[1] == 0;
+    return x;
 }
 
 // Copy / prefetch descriptors held by the lanes of warp 0 (at most 2 each): pointer for
@@ -229,7 +283,9 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     double a1[5], a2[5], s1[5], e1[5], aR1[5], Fp[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
+    const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
 
+    int next_issue = D;          // first step whose copies have not been issued (warp 0)
 _Pragma(RING_STR(unroll RING_UNROLL))
     for (int it = 0; it < nsteps; ++it) {
         const int n = m0 - 3 + it;
@@ -295,6 +351,22 @@ _Pragma(RING_STR(unroll RING_UNROLL))
 #pragma unroll
                         for (int c = 0; c < 5; ++c) a.Uout[zo + c * g.cstride] = un[c];
                         a.Uout[zo + 5 * g.cstride] = re;
+                        if (xe.single) {
+                            const long long zi = zo + xe.d[0];
+#pragma unroll
+                            for (int c = 0; c < 5; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && xe.f[0]) ? -un[c] : un[c];
+                            a.Uout[zi + 5 * g.cstride] = re;
+                        } else if (xe.any) {
+#pragma unroll 1
+                            for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
+                                const int q = qr < xe.n[0] ? 0 : 1, r = qr - (q ? xe.n[0] : 0);
+                                const long long zi = zo + (q ? xe.d[1] : xe.d[0]) + r * (q ? xe.step[1] : xe.step[0]);
+                                const bool fq = q ? xe.f[1] : xe.f[0];
+#pragma unroll
+                                for (int c = 0; c < 5; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && fq) ? -un[c] : un[c];
+                                a.Uout[zi + 5 * g.cstride] = re;
+                            }
+                        }
                     }
                 }
             }
@@ -302,7 +374,24 @@ _Pragma(RING_STR(unroll RING_UNROLL))
             for (int c = 0; c < 5; ++c) Fp[c] = F[c];
         }
         // release slot (it-KEEP); warp 0 refills the slot released one step earlier
-#if RING_CTASYNC
+#if RING_CTASYNC == 2
+        // Slot release without a CTA-wide barrier: every warp arrives on the slot's "empty"
+        // mbarrier; warp 0 refills whatever slots have been released by all warps (non-blocking
+        // test), and blocks only if the step it needs next has not been issued yet.
+        if (it >= KEEP) {
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
+        }
+        if (tid < 32) {
+            while (next_issue < nsteps) {
+                const int rel = next_issue - D;
+                if (next_issue <= it + 1) mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
+                else if (!mbar_test_warp(&empty[rel % D], (uint32_t)((rel / D) & 1))) break;
+                issue(next_issue);
+                ++next_issue;
+            }
+        }
+#elif RING_CTASYNC
         __syncthreads();
         if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
 #else
@@ -414,10 +503,12 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     double a1[NS], a2[NS], s1[NS], e1[NS], aR1[NS], Fp[NS];
 #pragma unroll
     for (int v = 0; v < NS; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
+    const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
     // F_rho of the face handled at step `it` is loaded one step ahead (ncu r01: 23-25 % of this
     // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
     double Fnext = 0.0;
 
+    int next_issue = D;          // first step whose copies have not been issued (warp 0)
 _Pragma(RING_STR(unroll RING_UNROLL))
     for (int it = 0; it < nsteps; ++it) {
         const int n = m0 - 3 + it;
@@ -454,19 +545,55 @@ _Pragma(RING_STR(unroll RING_UNROLL))
         }
         // pass 2: accumulator / stage update (first use of this step's global loads)
         if (upd) {
+            if (!FINAL) {
 #pragma unroll
-            for (int v = 0; v < NS; ++v) {
-                const double L = lacc[v] - dF[v] * dinv;
-                if (!FINAL) {
+                for (int v = 0; v < NS; ++v) {
+                    const double L = lacc[v] - dF[v] * dinv;
                     if (m.active) Lb[z * lmstride + v * g.lcstride] = L;
-                } else {
+                }
+            } else {
+                double un[NS];
+                const long long zo = zo0 + z * mstride;
+#pragma unroll
+                for (int v = 0; v < NS; ++v) {
+                    const double L = lacc[v] - dF[v] * dinv;
                     const double us = sz[(1 + v) * BS + tid];
-                    const double un = rk_combine<STAGE>(us, (STAGE == 1) ? ubase[v] : 0.0, dt, L);
-                    if (m.active) a.Uout[zo0 + z * mstride + v * g.cstride] = un;
+                    un[v] = rk_combine<STAGE>(us, (STAGE == 1) ? ubase[v] : 0.0, dt, L);
+                    if (m.active) a.Uout[zo + v * g.cstride] = un[v];
+                }
+                if (xe.single) {     // x ghost images of the zone (only the threads at the row ends)
+                    const long long zi = zo + xe.d[0];
+#pragma unroll
+                    for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = un[v];
+                } else if (xe.any) {
+#pragma unroll 1
+                    for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
+                        const int q = qr < xe.n[0] ? 0 : 1, r = qr - (q ? xe.n[0] : 0);
+                        const long long zi = zo + (q ? xe.d[1] : xe.d[0]) + r * (q ? xe.step[1] : xe.step[0]);
+#pragma unroll
+                        for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = un[v];
+                    }
                 }
             }
         }
-#if RING_CTASYNC
+#if RING_CTASYNC == 2
+        // Slot release without a CTA-wide barrier: every warp arrives on the slot's "empty"
+        // mbarrier; warp 0 refills whatever slots have been released by all warps (non-blocking
+        // test), and blocks only if the step it needs next has not been issued yet.
+        if (it >= KEEP) {
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
+        }
+        if (tid < 32) {
+            while (next_issue < nsteps) {
+                const int rel = next_issue - D;
+                if (next_issue <= it + 1) mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
+                else if (!mbar_test_warp(&empty[rel % D], (uint32_t)((rel / D) & 1))) break;
+                issue(next_issue);
+                ++next_issue;
+            }
+        }
+#elif RING_CTASYNC
         __syncthreads();
         if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
 #else

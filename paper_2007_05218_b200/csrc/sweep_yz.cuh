@@ -27,6 +27,7 @@ struct SweepArgs {
     double dt;             // host dt when dt_dev == nullptr
     int seglen;            // zones per pencil segment along DIR
     int sbase;             // first species of this launch (species kernels)
+    int xends;             // FINAL ring kernels: also write the x-direction ghost images of every zone
 };
 
 // pencil decode shared by both kernels.  Returns false if the thread has no pencil.
