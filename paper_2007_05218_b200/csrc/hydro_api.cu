@@ -50,6 +50,7 @@ struct hydro_ctx {
     int ns_max;
     bool use_ring;            // TMA-ring marching kernels usable for this geometry
     bool split_ghosts;        // hydro_step: x ghost images written by the z sweeps + ghost-row copies
+    CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs on the handle's stream
     bool profiling;
@@ -123,6 +124,37 @@ Carve carve(const Geom &g)
     return c;
 }
 
+// TMA view of one state for the ring kernels of direction dir (1: y march, 2: z march): a 5-D
+// tensor (i, j, k, component, box) with a box of W zones x R rows x nc components, R counted
+// along the transverse dimension (k for the y march, j for the z march).
+bool make_ring_map(CUtensorMap *out, double *U, const Geom &g, int dir, int nc, std::string &why)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+            why = "cuTensorMapEncodeTiled is not available from the driver";
+            return false;
+        }
+        encode = (encode_fn)fn;
+    }
+    const int W = g.nb[0] < BS ? g.nb[0] : BS, R = BS / W;
+    cuuint64_t dims[5] = {(cuuint64_t)g.nt[0], (cuuint64_t)g.nt[1], (cuuint64_t)g.nt[2], (cuuint64_t)g.nvar,
+                          (cuuint64_t)g.nboxes};
+    cuuint64_t strides[4] = {(cuuint64_t)g.nt[0] * 8, (cuuint64_t)g.nt[0] * g.nt[1] * 8, (cuuint64_t)g.cstride * 8,
+                             (cuuint64_t)g.bstride * 8};
+    cuuint32_t box[5] = {(cuuint32_t)W, dir == 2 ? (cuuint32_t)R : 1u, dir == 1 ? (cuuint32_t)R : 1u, (cuuint32_t)nc, 1u};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
 int fail(hydro_handle h, int code, const std::string &msg)
 {
     if (h) h->err = msg; else g_init_error = msg;
@@ -173,14 +205,17 @@ void set_smem(K kernel, size_t bytes)
 }
 
 template <int DIR, bool FINAL, int STAGE>
-void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
+void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, int state)
 {
+    RingMaps tm;
+    tm.a = h->maps[state][DIR - 1][1];
+    tm.b = h->maps[state][DIR - 1][ns];
     switch (ns) {
 #define CASE(N) case N: { \
-        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + 2 * RING_D * 8 + sizeof(RingDesc); \
+        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + RING_D * 8; \
         auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D>; \
         static bool once = (set_smem(kern, sm), true); (void)once; \
-        kern<<<grid, BS, sm, h->stream>>>(h->g, a); } break;
+        kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } break;
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
         default: break;
@@ -199,7 +234,7 @@ void launch_species(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
 }
 
 template <int DIR, bool FINAL, int STAGE>
-int sweep_dir(hydro_handle h, SweepArgs a)
+int sweep_dir(hydro_handle h, SweepArgs a, int state)
 {
     const Geom &g = h->g;
     constexpr int T = DIR == 1 ? 2 : 1;
@@ -214,10 +249,13 @@ int sweep_dir(hydro_handle h, SweepArgs a)
     prof_begin(h);
     if (ring) {
         constexpr int NROW = FINAL ? 6 : 5;
-        const size_t sm = (size_t)RING_D * NROW * BS * 8 + 2 * RING_D * 8 + sizeof(RingDesc);
+        const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
         auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D>;
         static bool once = (set_smem(kern, sm), true); (void)once;
-        kern<<<grid, BS, sm, h->stream>>>(g, a);
+        RingMaps tm;
+        tm.a = h->maps[state][DIR - 1][FINAL ? 6 : 4];
+        tm.b = h->maps[state][DIR - 1][1];
+        kern<<<grid, BS, sm, h->stream>>>(g, a, tm);
     } else
         k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
@@ -230,7 +268,7 @@ int sweep_dir(hydro_handle h, SweepArgs a)
             const int ns = base + (gr < rem ? 1 : 0);
             a.sbase = s0;
             prof_begin(h);
-            if (ring) launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid);
+            if (ring) launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid, state);
             else launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
             if ((rc = check_launch(h, "k_sweep_species", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
             s0 += ns;
@@ -263,10 +301,10 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
         int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }
-    int rc = sweep_dir<1, false, 0>(h, a);
+    int rc = sweep_dir<1, false, 0>(h, a, stage);
     if (rc) return rc;
-    if (stage == 0) return sweep_dir<2, true, 0>(h, a);
-    return sweep_dir<2, true, 1>(h, a);
+    if (stage == 0) return sweep_dir<2, true, 0>(h, a, stage);
+    return sweep_dir<2, true, 1>(h, a, stage);
 }
 
 int fill_ghosts_impl(hydro_handle h, int which)
@@ -351,12 +389,17 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     const char *env = getenv("HYDRO_NSMAX");
     h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
-    {   // TMA bulk copies need 16-byte aligned row segments that tile the CTA exactly
+    {   // TMA tensor copies: 16-byte row pitch, row segments that tile the CTA exactly, at most nvar-deep boxes
         const int W = g.nb[0] < BS ? g.nb[0] : BS;
         const char *er = getenv("HYDRO_RING");
-        // and at most 64 copies per march step (2 descriptors per lane of warp 0): W >= 16
-        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && (W >= 16) &&
-                      !(er && atoi(er) == 0);
+        h->use_ring = (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && !(er && atoi(er) == 0);
+        for (int st = 0; st < 2 && h->use_ring; ++st)
+            for (int dir = 1; dir <= 2 && h->use_ring; ++dir)
+                for (int nc = 1; nc <= 6 && h->use_ring; ++nc) {
+                    if (nc > g.nvar) continue;
+                    std::string why2;
+                    if (!make_ring_map(&h->maps[st][dir - 1][nc], h->U[st], g, dir, nc, why2)) h->use_ring = false;
+                }
     }
     {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
         const char *ef = getenv("HYDRO_SPLIT_GHOSTS");

@@ -1,43 +1,34 @@
-// march_ring.cuh -- y/z marching sweeps fed by a TMA bulk-copy ring in shared memory.
+// march_ring.cuh -- y/z marching sweeps fed by a TMA tensor-copy ring in shared memory.
 //
 // Same arithmetic and accumulator protocol as sweep_yz.cuh (the generic fallback); what
 // changes is how zones reach the registers.  A CTA of BS threads owns BS pencils laid out
-// as R row segments of W contiguous zones.  For every march step one elected set of
-// threads issues cp.async.bulk (TMA, 1-D) copies of the step's rows -- W*8 contiguous
-// bytes per component per row segment -- into slot (step % D) of a D-deep ring, signalled
-// through a "full" mbarrier with an expected-bytes count.  The copies run D-KEEP-1 steps
-// ahead of the arithmetic, so the bytes in flight per SM are set by the ring depth and not
-// by how many registers a thread can spare: that is what the y/z sweeps lacked (ncu: 17 %
-// occupancy, fp64 pipe 19-30 %, DRAM 25-35 % of peak with plain per-thread loads).
-// Slot reuse is ordered by one __syncthreads per step (RING_CTASYNC=1, measured faster than
-// per-warp "empty" mbarriers, RING_CTASYNC=0).  The accumulator / face-flux / U0 rows that the
-// update needs are read with plain loads issued at the top of the step; pulling them into L2
-// ahead of time with cp.async.bulk.prefetch.L2 (RING_PF=1) measured slower and is off.
-// FINAL (z) kernels keep the last KEEP=3 slots alive so that the update of zone n-3 reads
-// its raw conserved state from shared memory instead of going back to L2.
+// as R row segments of W contiguous zones (R consecutive rows of the plane normal to DIR).
+// For every march step ONE thread issues one or two cp.async.bulk.tensor copies (TMA, 5-D
+// tiled tensor map over a state: i, j, k, component, box; SASS UTMALDG) that bring the
+// step's rows of all components the kernel reads -- a {W, R, NC} box -- into slot
+// (step % D) of a D-deep ring, signalled through a "full" mbarrier with an expected-bytes
+// count.  The copies run D-KEEP-1 steps ahead of the arithmetic, so the bytes in flight per
+// SM are set by the ring depth and not by how many registers a thread can spare.  Slot reuse
+// is ordered by one __syncthreads per step.  FINAL (z) kernels keep the last KEEP = 3 slots
+// alive so that the update of zone n-3 reads its raw conserved state from shared memory.
+//
+// Measured dead ends (profiles/r01_experiments.md): per-row 1-D bulk copies issued by the 32
+// lanes of warp 0 (ptxas serialises them through ELECT loops: ~10 instructions per copy on the
+// critical warp); per-warp "empty" mbarriers instead of the CTA barrier, blocking or polled;
+// L2 prefetch of the accumulator rows; the accumulator rows through the ring; unroll by 2.
 #pragma once
+#include <cuda.h>
+
 #include "hydro_device.cuh"
 #include "sweep_yz.cuh"
 #include "ghost_reduce.cuh"
 
-// tuning switches (overridable with -D for experiments)
-#ifndef RING_UNROLL
-#define RING_UNROLL 1      // unroll factor of the march loop
-#endif
-#ifndef RING_PF
-#define RING_PF 0          // cp.async.bulk.prefetch.L2 of the accumulator / face-flux / U0 rows
-#endif
-#ifndef RING_CTASYNC
-#define RING_CTASYNC 1     // 1: __syncthreads per step instead of per-warp slot release
-#endif
 #ifndef RING_MINB
 #define RING_MINB 3        // CTAs per SM the hydro kernels' register allocation is capped for
 #endif
 #ifndef RING_MINB_S
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
-#define RING_STR2(x) #x
-#define RING_STR(x) RING_STR2(x)
 
 namespace hydro {
 
@@ -58,19 +49,18 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+// 5-D tiled tensor copy global -> shared, completion on an mbarrier (coordinates innermost first)
+__device__ __forceinline__ void tma_load_5d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2,
+                                            int c3, int c4)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
+    asm volatile(
+        "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
+        : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map)
 {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
@@ -86,26 +76,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
         : "memory");
 }
 
-// non-blocking phase test by lane 0, broadcast to the warp
-__device__ __forceinline__ bool mbar_test_warp(uint64_t* bar, uint32_t parity)
-{
-    uint32_t ok = 0;
-    if ((threadIdx.x & 31) == 0) {
-        asm volatile(
-            "{\n"
-            ".reg .pred P1;\n"
-            "mbarrier.test_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, P1;\n"
-            "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    }
-    return __shfl_sync(0xffffffffu, ok, 0) != 0;
-}
+// The two tensor maps of a launch (built on the host, hydro_api.cu): `a` and `b` view the
+// stage state with boxes {W, R rows, NCa components} and {W, R rows, NCb components}.
+struct RingMaps {
+    CUtensorMap a, b;
+};
 
 // Decomposition of a CTA into R row segments of W zones.
 struct RingMap {
     int W, R;        // zones per row segment, row segments per CTA
     int r, ii;       // this thread's row segment and position in it
     int i, t;        // pencil coordinates (t clamped into range)
+    int x0, t0;      // first zone / first row of the CTA's tile
     bool active;     // pencil exists (t in range)
 };
 
@@ -118,14 +100,15 @@ __device__ __forceinline__ RingMap ring_map(const Geom& g, int tid, int cta)
     m.R = BS / m.W;
     m.r = tid / m.W;
     m.ii = tid - m.r * m.W;
-    const int xchunks = g.nb[0] / m.W;
-    const int rc = cta * m.R + m.r;
-    int t = rc / xchunks;
-    const int xc = rc - t * xchunks;
+    const int xchunks = g.nb[0] / m.W;       // > 1 only when W == BS (R == 1)
+    const int rc0 = cta * m.R;
+    m.t0 = rc0 / xchunks;
+    m.x0 = (rc0 - m.t0 * xchunks) * m.W;
+    int t = m.t0 + m.r;
     m.active = t < g.nb[T];
     if (!m.active) t = g.nb[T] - 1;
     m.t = t;
-    m.i = xc * m.W + m.ii;
+    m.i = m.x0 + m.ii;
     return m;
 }
 
@@ -145,6 +128,14 @@ __device__ __forceinline__ long long flat_off(const Geom& g, int i, int t, int n
     return (DIR == 1) ? ((long long)t * ext + n) * g.nb[0] + i : ((long long)n * g.nb[1] + t) * g.nb[0] + i;
 }
 
+// issue the tensor copy of march step `it` (one thread): rows of zone index n = m0-3+it
+template <int DIR>
+__device__ __forceinline__ void ring_issue(const Geom& g, const RingMap& m, const CUtensorMap* map, void* dst,
+                                           uint64_t* bar, int n, int comp0, int box)
+{
+    const int j = (DIR == 1) ? n : m.t0, k = (DIR == 1) ? m.t0 : n;
+    tma_load_5d(dst, map, bar, m.x0 + g.ng, j + g.ng, k + g.ng, comp0, box);
+}
 
 // x-direction ghost images of this thread's pencil (FINAL kernels with a.xends).  With boxes
 // at least ng wide a zone has at most two groups of images, one per side; a group is a single
@@ -160,53 +151,43 @@ struct XEnds {
 };
 __device__ __forceinline__ XEnds xends_setup(const Geom& g, bool on, int b, int i)
 {
-    XEnds x;
-    x.d[0] = x.d[1] = 0; x.n[0] = x.n[1] = 0; x.step[0] = x.step[1] = 1; x.f[0] = x.f[1] = false;
+    // scalars only (no dynamically indexed arrays: the struct must stay in registers)
+    long long d0 = 0, d1 = 0;
+    int n0 = 0, n1 = 0, st0 = 1, st1 = 1;
+    bool f0 = false, f1 = false;
     if (on) {
         const int bi = b % g.NB[0];
-        int db, p, q = 0, grp = -1, ldb = 0, lp = 0;
+        int db, p, q = 0, ldb = 0, lp = 0;
         bool f;
         while (dim_image(g, 0, bi, i, q, db, p, f)) {
-            const bool run = grp >= 0 && db == ldb && f == x.f[grp] && (p == lp + 1 || p == lp - 1) &&
-                             (x.n[grp] == 1 || p - lp == x.step[grp]);
-            if (run) { x.step[grp] = p - lp; ++x.n[grp]; }
-            else if (grp < 1) {
-                ++grp;
-                x.d[grp] = (long long)(db - bi) * g.bstride + (p - (i + g.ng));
-                x.n[grp] = 1; x.f[grp] = f;
-            }
+            const bool adj = q > 0 && db == ldb && (p == lp + 1 || p == lp - 1);
+            if (n1 == 0 && n0 > 0 && adj && f == f0 && (n0 == 1 || p - lp == st0)) { st0 = p - lp; ++n0; }
+            else if (n1 > 0 && adj && f == f1 && (n1 == 1 || p - lp == st1)) { st1 = p - lp; ++n1; }
+            else if (n0 == 0) { d0 = (long long)(db - bi) * g.bstride + (p - (i + g.ng)); n0 = 1; f0 = f; }
+            else if (n1 == 0) { d1 = (long long)(db - bi) * g.bstride + (p - (i + g.ng)); n1 = 1; f1 = f; }
             ldb = db; lp = p; ++q;
         }
     }
-    x.any = (x.n[0] | x.n[1]) != 0;
-    x.single = x.n[0] == 1 && x.n[1] == 0;
+    XEnds x;
+    x.d[0] = d0; x.d[1] = d1; x.n[0] = n0; x.n[1] = n1; x.step[0] = st0; x.step[1] = st1; x.f[0] = f0; x.f[1] = f1;
+    x.any = (n0 | n1) != 0;
+    x.single = n0 == 1 && n1 == 0;
     return x;
 }
 
-// Copy / prefetch descriptors held by the lanes of warp 0 (at most 2 each): pointer for
-// march step 0 and the destination offset inside a ring slot (copies), or the first step at
-// which the row exists (prefetches).  Per step a lane only adds step*stride.
-struct RingDesc {          // lives in shared memory: entry q*32 + lane
-    const double* src[64];
-    const double* pf[64];
-    long long pf_stride[64];
-    int dst[64];
-    int pf_first[64];
-};
-
 // ------------------------------------------------------------------------------------
+// hydro variables.  Ring rows: non-FINAL  rho, mx, my, mz (map a, 4 components) + rho*e (map b,
+// 1 component); FINAL  rho, mx, my, mz, rho*E, rho*e (map a, 6 components).
 template <int DIR, bool FINAL, int STAGE, int BS, int D>
 __global__ void __launch_bounds__(BS, RING_MINB)
-k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
+k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
-    constexpr int T = (DIR == 1) ? 2 : 1;
     constexpr int NROW = FINAL ? 6 : 5;
     constexpr int KEEP = FINAL ? 3 : 0;
-    constexpr int NPF = 5 + ((FINAL && STAGE == 1) ? 5 : 0);        // Lacc rows (+ U0 rows)
+    constexpr int ROW_E = FINAL ? 5 : 4;       // ring row of rho*e
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
-    uint64_t* empty = full + D;
 
     const int tid = threadIdx.x;
     const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
@@ -214,69 +195,34 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     const int m0 = blockIdx.y * a.seglen;
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
-    const double* Ub = a.Us + (long long)b * g.bstride;
     const long long mstride = (DIR == 1) ? g.nt[0] : (long long)g.nt[0] * g.nt[1];
     const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
-    double* Lbox = a.Lacc + (long long)b * g.lbstride;
 
-    RingDesc& ds = *reinterpret_cast<RingDesc*>(empty + D);
-    if (tid < 32) {
-        const int xchunks = g.nb[0] / m.W;
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const int cpy = tid + 32 * q;
-            ds.src[q * 32 + tid] = nullptr; ds.dst[q * 32 + tid] = 0; ds.pf[q * 32 + tid] = nullptr; ds.pf_first[q * 32 + tid] = 0; ds.pf_stride[q * 32 + tid] = 0;
-            const int row = cpy / m.R, r = cpy - row * m.R;
-            const int rc = blockIdx.x * m.R + r;
-            int t = rc / xchunks;
-            const int x0 = (rc - t * xchunks) * m.W;
-            if (t >= g.nb[T]) t = g.nb[T] - 1;
-            if (row < NROW) {
-                const int comp = row < 4 ? row : (row == 4 ? 5 : 4);   // rho, mx, my, mz, rho*e, (rho*E)
-                ds.src[q * 32 + tid] = Ub + (long long)comp * g.cstride + zone_off<DIR>(g, x0, t, m0 - 3);
-                ds.dst[q * 32 + tid] = row * BS + r * m.W;
-            }
-            if (row < NPF) {     // row of zone n-3 = m0-6+it: exists from step 6 on
-                ds.pf_first[q * 32 + tid] = 6;
-                if (row < 5) {
-                    ds.pf[q * 32 + tid] = Lbox + (long long)row * g.lcstride + flat_off<DIR>(g, x0, t, m0 - 6, g.nb[DIR]);
-                    ds.pf_stride[q * 32 + tid] = lmstride;
-                } else {
-                    ds.pf[q * 32 + tid] = a.Ubase + (long long)b * g.bstride + (long long)(row - 5) * g.cstride +
-                               zone_off<DIR>(g, x0, t, m0 - 6);
-                    ds.pf_stride[q * 32 + tid] = mstride;
-                }
-            }
-        }
-    }
-    auto issue = [&](int it) {      // warp 0 only
+    auto issue = [&](int it) {      // thread 0 only
         uint64_t* bar = &full[it % D];
         double* slot = ring + (size_t)(it % D) * NROW * BS;
-        if (tid == 0) mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const double* src = ds.src[q * 32 + tid];
-            if (src) bulk_g2s(slot + ds.dst[q * 32 + tid], src + it * mstride, (uint32_t)(m.W * 8), bar);
-#if RING_PF
-            const double* pf = ds.pf[q * 32 + tid];
-            if (pf && it >= ds.pf_first[q * 32 + tid])
-                bulk_prefetch_l2(pf + it * ds.pf_stride[q * 32 + tid], (uint32_t)(m.W * 8));
-#endif
+        mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
+        if (FINAL) ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
+        else {
+            ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
+            ring_issue<DIR>(g, m, &tm.b, slot + 4 * BS, bar, m0 - 3 + it, 5, b);
         }
     };
 
     if (tid == 0) {
-        for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BS / 32); }
+        tma_prefetch_desc(&tm.a);
+        if (!FINAL) tma_prefetch_desc(&tm.b);
+        for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid < 32)
+    if (tid == 0)
         for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
-    double* Lb = Lbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR]);
-    double* Fb = a.Frho + (long long)b * g.fbstride + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR] + 1);
-    const long long zo0 = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, 0);
+    // running offsets of zone z = m0-6+it (the zone updated at step it) and of face n-2
+    long long lz = (long long)b * g.lbstride + flat_off<DIR>(g, m.i, m.t, m0 - 6, g.nb[DIR]);
+    long long fz = (long long)b * g.fbstride + flat_off<DIR>(g, m.i, m.t, m0 - 5, g.nb[DIR] + 1);
+    long long zo = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, m0 - 6);
     const double dinv = g.dxinv[DIR];
     const double dt = a.dt_dev ? *a.dt_dev : a.dt;
 
@@ -285,26 +231,22 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
     const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
 
-    int next_issue = D;          // first step whose copies have not been issued (warp 0)
-_Pragma(RING_STR(unroll RING_UNROLL))
-    for (int it = 0; it < nsteps; ++it) {
-        const int n = m0 - 3 + it;
-        const int z = n - 3;
+    for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
-        // early, independent global loads for the update of zone z (L2 hits: prefetched by warp 0)
+        // early, independent global loads for the update of zone z
         double lacc[5], ubase[5];
         if (upd) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) lacc[c] = Lb[z * lmstride + c * g.lcstride];
+            for (int c = 0; c < 5; ++c) lacc[c] = a.Lacc[lz + c * g.lcstride];
             if (FINAL && STAGE == 1) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) ubase[c] = a.Ubase[zo0 + z * mstride + c * g.cstride];
+                for (int c = 0; c < 5; ++c) ubase[c] = a.Ubase[zo + c * g.cstride];
             }
         }
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         double q[5], rinv;
-        cons_to_prim(g, slot[tid], slot[BS + tid], slot[2 * BS + tid], slot[3 * BS + tid], slot[4 * BS + tid], q, rinv);
+        cons_to_prim(g, slot[tid], slot[BS + tid], slot[2 * BS + tid], slot[3 * BS + tid], slot[ROW_E * BS + tid], q, rinv);
         double qL[5], qR[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -319,52 +261,50 @@ _Pragma(RING_STR(unroll RING_UNROLL))
         if (it >= 5) {
             double F[5];
             hllc<DIR>(g, qL, qR, F);
-            if (m.active) Fb[(long long)(n - 2) * lmstride] = F[0];
+            double out[6];
             if (upd) {
-                if (!FINAL) {
-                    if (m.active) {
 #pragma unroll
-                        for (int c = 0; c < 5; ++c) Lb[z * lmstride + c * g.lcstride] = lacc[c] - (F[c] - Fp[c]) * dinv;
-                    }
-                } else {
-                    double L[5];
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) L[c] = lacc[c] - (F[c] - Fp[c]) * dinv;
+                for (int c = 0; c < 5; ++c) out[c] = lacc[c] - (F[c] - Fp[c]) * dinv;
+                if (FINAL) {
                     const double* sz = ring + (size_t)((it - 3) % D) * NROW * BS;   // raw state of zone z
                     double us[5];
                     us[0] = sz[tid]; us[1] = sz[BS + tid]; us[2] = sz[2 * BS + tid]; us[3] = sz[3 * BS + tid];
-                    us[4] = sz[5 * BS + tid];
+                    us[4] = sz[4 * BS + tid];
                     if (g.has_grav) {
-                        L[1] += us[0] * g.grav[0];
-                        L[2] += us[0] * g.grav[1];
-                        L[3] += us[0] * g.grav[2];
-                        L[4] += us[1] * g.grav[0] + us[2] * g.grav[1] + us[3] * g.grav[2];
+                        out[1] += us[0] * g.grav[0];
+                        out[2] += us[0] * g.grav[1];
+                        out[3] += us[0] * g.grav[2];
+                        out[4] += us[1] * g.grav[0] + us[2] * g.grav[1] + us[3] * g.grav[2];
                     }
-                    double un[5];
 #pragma unroll
-                    for (int c = 0; c < 5; ++c) un[c] = rk_combine<STAGE>(us[c], (STAGE == 1) ? ubase[c] : 0.0, dt, L[c]);
-                    const double K = ddiv(HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]), un[0]);
-                    double re = un[4] - K;
+                    for (int c = 0; c < 5; ++c) out[c] = rk_combine<STAGE>(us[c], (STAGE == 1) ? ubase[c] : 0.0, dt, out[c]);
+                    const double K = ddiv(HALF * (out[1] * out[1] + out[2] * out[2] + out[3] * out[3]), out[0]);
+                    double re = out[4] - K;
                     if (re < g.floor_rhoe) re = g.floor_rhoe;
-                    if (m.active) {
-                        const long long zo = zo0 + z * mstride;
+                    out[5] = re;
+                }
+            }
+            if (m.active) {          // all stores of the step under one predicate
+                a.Frho[fz] = F[0];
+                if (upd) {
+                    if (!FINAL) {
 #pragma unroll
-                        for (int c = 0; c < 5; ++c) a.Uout[zo + c * g.cstride] = un[c];
-                        a.Uout[zo + 5 * g.cstride] = re;
+                        for (int c = 0; c < 5; ++c) a.Lacc[lz + c * g.lcstride] = out[c];
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) a.Uout[zo + c * g.cstride] = out[c];
                         if (xe.single) {
                             const long long zi = zo + xe.d[0];
 #pragma unroll
-                            for (int c = 0; c < 5; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && xe.f[0]) ? -un[c] : un[c];
-                            a.Uout[zi + 5 * g.cstride] = re;
+                            for (int c = 0; c < 6; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && xe.f[0]) ? -out[c] : out[c];
                         } else if (xe.any) {
 #pragma unroll 1
                             for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
-                                const int q = qr < xe.n[0] ? 0 : 1, r = qr - (q ? xe.n[0] : 0);
-                                const long long zi = zo + (q ? xe.d[1] : xe.d[0]) + r * (q ? xe.step[1] : xe.step[0]);
-                                const bool fq = q ? xe.f[1] : xe.f[0];
+                                const int qq = qr < xe.n[0] ? 0 : 1, r = qr - (qq ? xe.n[0] : 0);
+                                const long long zi = zo + (qq ? xe.d[1] : xe.d[0]) + r * (qq ? xe.step[1] : xe.step[0]);
+                                const bool fq = qq ? xe.f[1] : xe.f[0];
 #pragma unroll
-                                for (int c = 0; c < 5; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && fq) ? -un[c] : un[c];
-                                a.Uout[zi + 5 * g.cstride] = re;
+                                for (int c = 0; c < 6; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && fq) ? -out[c] : out[c];
                             }
                         }
                     }
@@ -373,56 +313,24 @@ _Pragma(RING_STR(unroll RING_UNROLL))
 #pragma unroll
             for (int c = 0; c < 5; ++c) Fp[c] = F[c];
         }
-        // release slot (it-KEEP); warp 0 refills the slot released one step earlier
-#if RING_CTASYNC == 2
-        // Slot release without a CTA-wide barrier: every warp arrives on the slot's "empty"
-        // mbarrier; warp 0 refills whatever slots have been released by all warps (non-blocking
-        // test), and blocks only if the step it needs next has not been issued yet.
-        if (it >= KEEP) {
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
-        }
-        if (tid < 32) {
-            while (next_issue < nsteps) {
-                const int rel = next_issue - D;
-                if (next_issue <= it + 1) mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
-                else if (!mbar_test_warp(&empty[rel % D], (uint32_t)((rel / D) & 1))) break;
-                issue(next_issue);
-                ++next_issue;
-            }
-        }
-#elif RING_CTASYNC
+        // release slot (it-KEEP): one CTA barrier per step, then thread 0 refills it
         __syncthreads();
-        if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
-#else
-        if (it >= KEEP) {
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
-        }
-        if (tid < 32) {
-            const int rel = it - KEEP - 1;
-            if (rel >= 0 && rel + D < nsteps) {
-                mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
-                issue(rel + D);
-            }
-        }
-#endif
+        if (tid == 0 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
     }
 }
 
 // ------------------------------------------------------------------------------------
+// NS passive species per thread.  Ring rows: rho (map a, 1 component) + rho*X_k, k = sbase..
+// sbase+NS-1 (map b, NS components).
 template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D>
 __global__ void __launch_bounds__(BS, RING_MINB_S)
-k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
+k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
-    constexpr int T = (DIR == 1) ? 2 : 1;
     constexpr int NROW = 1 + NS;
     constexpr int KEEP = FINAL ? 3 : 0;
-    constexpr int NPF = 1 + NS + ((FINAL && STAGE == 1) ? NS : 0);  // F_rho, Lacc rows (+ U0 rows)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
-    uint64_t* empty = full + D;
 
     const int tid = threadIdx.x;
     const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
@@ -431,72 +339,31 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
     const int sbase = a.sbase;
-    const double* Ub = a.Us + (long long)b * g.bstride;
     const long long mstride = (DIR == 1) ? g.nt[0] : (long long)g.nt[0] * g.nt[1];
     const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
-    double* Lbox = a.Lacc + (long long)b * g.lbstride + (long long)(5 + sbase) * g.lcstride;
-    const double* Fbox = a.Frho + (long long)b * g.fbstride;
 
-    RingDesc& ds = *reinterpret_cast<RingDesc*>(empty + D);
-    if (tid < 32) {
-        const int xchunks = g.nb[0] / m.W;
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const int cpy = tid + 32 * q;
-            ds.src[q * 32 + tid] = nullptr; ds.dst[q * 32 + tid] = 0; ds.pf[q * 32 + tid] = nullptr; ds.pf_first[q * 32 + tid] = 0; ds.pf_stride[q * 32 + tid] = 0;
-            const int row = cpy / m.R, r = cpy - row * m.R;
-            const int rc = blockIdx.x * m.R + r;
-            int t = rc / xchunks;
-            const int x0 = (rc - t * xchunks) * m.W;
-            if (t >= g.nb[T]) t = g.nb[T] - 1;
-            if (row < NROW) {
-                const int comp = row == 0 ? 0 : 5 + sbase + row;       // rho, then rho*X_k
-                ds.src[q * 32 + tid] = Ub + (long long)comp * g.cstride + zone_off<DIR>(g, x0, t, m0 - 3);
-                ds.dst[q * 32 + tid] = row * BS + r * m.W;
-            }
-            if (row < NPF) {
-                if (row == 0) {          // F_rho of face n-2 = m0-5+it: exists from step 5 on
-                    ds.pf[q * 32 + tid] = Fbox + flat_off<DIR>(g, x0, t, m0 - 5, g.nb[DIR] + 1);
-                    ds.pf_first[q * 32 + tid] = 5; ds.pf_stride[q * 32 + tid] = lmstride;
-                } else if (row <= NS) {  // Lacc of zone n-3
-                    ds.pf[q * 32 + tid] = Lbox + (long long)(row - 1) * g.lcstride + flat_off<DIR>(g, x0, t, m0 - 6, g.nb[DIR]);
-                    ds.pf_first[q * 32 + tid] = 6; ds.pf_stride[q * 32 + tid] = lmstride;
-                } else {                 // U0 rho*X_k of zone n-3
-                    ds.pf[q * 32 + tid] = a.Ubase + (long long)b * g.bstride + (long long)(6 + sbase + row - 1 - NS) * g.cstride +
-                               zone_off<DIR>(g, x0, t, m0 - 6);
-                    ds.pf_first[q * 32 + tid] = 6; ds.pf_stride[q * 32 + tid] = mstride;
-                }
-            }
-        }
-    }
-    auto issue = [&](int it) {      // warp 0 only
+    auto issue = [&](int it) {      // thread 0 only
         uint64_t* bar = &full[it % D];
         double* slot = ring + (size_t)(it % D) * NROW * BS;
-        if (tid == 0) mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
-        __syncwarp();
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {
-            const double* src = ds.src[q * 32 + tid];
-            if (src) bulk_g2s(slot + ds.dst[q * 32 + tid], src + it * mstride, (uint32_t)(m.W * 8), bar);
-#if RING_PF
-            const double* pf = ds.pf[q * 32 + tid];
-            if (pf && it >= ds.pf_first[q * 32 + tid])
-                bulk_prefetch_l2(pf + it * ds.pf_stride[q * 32 + tid], (uint32_t)(m.W * 8));
-#endif
-        }
+        mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
+        ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
+        ring_issue<DIR>(g, m, &tm.b, slot + BS, bar, m0 - 3 + it, 6 + sbase, b);
     };
 
     if (tid == 0) {
-        for (int s = 0; s < D; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], BS / 32); }
+        tma_prefetch_desc(&tm.a);
+        tma_prefetch_desc(&tm.b);
+        for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid < 32)
+    if (tid == 0)
         for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
-    double* Lb = Lbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR]);
-    const double* Fb = Fbox + flat_off<DIR>(g, m.i, m.t, 0, g.nb[DIR] + 1);
-    const long long zo0 = (long long)b * g.bstride + zone_off<DIR>(g, m.i, m.t, 0) + (long long)(6 + sbase) * g.cstride;
+    // running offsets of zone z = m0-6+it (updated at step it) and of face n-2 = m0-5+it
+    long long lz = (long long)b * g.lbstride + (long long)(5 + sbase) * g.lcstride + flat_off<DIR>(g, m.i, m.t, m0 - 6, g.nb[DIR]);
+    long long fz = (long long)b * g.fbstride + flat_off<DIR>(g, m.i, m.t, m0 - 5, g.nb[DIR] + 1);
+    long long zo = (long long)b * g.bstride + (long long)(6 + sbase) * g.cstride + zone_off<DIR>(g, m.i, m.t, m0 - 6);
     const double dinv = g.dxinv[DIR];
     const double dt = a.dt_dev ? *a.dt_dev : a.dt;
 
@@ -508,29 +375,24 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
     double Fnext = 0.0;
 
-    int next_issue = D;          // first step whose copies have not been issued (warp 0)
-_Pragma(RING_STR(unroll RING_UNROLL))
-    for (int it = 0; it < nsteps; ++it) {
-        const int n = m0 - 3 + it;
-        const int z = n - 3;
+    for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         const double Frho = Fnext;
-        if (it >= 4 && it + 1 < nsteps) Fnext = ldg(Fb + (long long)(n - 1) * lmstride);
+        if (it >= 4 && it + 1 < nsteps) Fnext = ldg(a.Frho + fz + lmstride);
         double lacc[NS], ubase[NS];
         if (upd) {
 #pragma unroll
-            for (int v = 0; v < NS; ++v) lacc[v] = Lb[z * lmstride + v * g.lcstride];
+            for (int v = 0; v < NS; ++v) lacc[v] = a.Lacc[lz + v * g.lcstride];
             if (FINAL && STAGE == 1) {
 #pragma unroll
-                for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo0 + z * mstride + v * g.cstride];
+                for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo + v * g.cstride];
             }
         }
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         const double rinv = drcp(dmax(slot[tid], g.small_dens));
-        const double* sz = ring + (size_t)((it + D - 3) % D) * NROW * BS;       // zone z's slot (FINAL)
         // pass 1: reconstruction and face fluxes of all NS species (no global operand)
-        double dF[NS];
+        double out[NS];
 #pragma unroll
         for (int v = 0; v < NS; ++v) {
             const double X = slot[(1 + v) * BS + tid] * rinv;
@@ -540,75 +402,44 @@ _Pragma(RING_STR(unroll RING_UNROLL))
             ppm_mono(e1[v], en, a2[v], aL, aR);
             const double Fs = Frho * (Frho >= 0.0 ? aR1[v] : aL);
             a2[v] = a1[v]; a1[v] = X; s1[v] = sn; e1[v] = en; aR1[v] = aR;
-            dF[v] = Fs - Fp[v];
+            out[v] = Fs - Fp[v];
             Fp[v] = Fs;
         }
         // pass 2: accumulator / stage update (first use of this step's global loads)
         if (upd) {
-            if (!FINAL) {
 #pragma unroll
-                for (int v = 0; v < NS; ++v) {
-                    const double L = lacc[v] - dF[v] * dinv;
-                    if (m.active) Lb[z * lmstride + v * g.lcstride] = L;
-                }
-            } else {
-                double un[NS];
-                const long long zo = zo0 + z * mstride;
+            for (int v = 0; v < NS; ++v) out[v] = lacc[v] - out[v] * dinv;
+            if (FINAL) {
+                const double* sz = ring + (size_t)((it + D - 3) % D) * NROW * BS;   // zone z's slot
 #pragma unroll
-                for (int v = 0; v < NS; ++v) {
-                    const double L = lacc[v] - dF[v] * dinv;
-                    const double us = sz[(1 + v) * BS + tid];
-                    un[v] = rk_combine<STAGE>(us, (STAGE == 1) ? ubase[v] : 0.0, dt, L);
-                    if (m.active) a.Uout[zo + v * g.cstride] = un[v];
-                }
-                if (xe.single) {     // x ghost images of the zone (only the threads at the row ends)
-                    const long long zi = zo + xe.d[0];
+                for (int v = 0; v < NS; ++v)
+                    out[v] = rk_combine<STAGE>(sz[(1 + v) * BS + tid], (STAGE == 1) ? ubase[v] : 0.0, dt, out[v]);
+            }
+            if (m.active) {          // all stores of the step under one predicate
+                if (!FINAL) {
 #pragma unroll
-                    for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = un[v];
-                } else if (xe.any) {
+                    for (int v = 0; v < NS; ++v) a.Lacc[lz + v * g.lcstride] = out[v];
+                } else {
+#pragma unroll
+                    for (int v = 0; v < NS; ++v) a.Uout[zo + v * g.cstride] = out[v];
+                    if (xe.single) {     // x ghost images of the zone (only the threads at the row ends)
+                        const long long zi = zo + xe.d[0];
+#pragma unroll
+                        for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = out[v];
+                    } else if (xe.any) {
 #pragma unroll 1
-                    for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
-                        const int q = qr < xe.n[0] ? 0 : 1, r = qr - (q ? xe.n[0] : 0);
-                        const long long zi = zo + (q ? xe.d[1] : xe.d[0]) + r * (q ? xe.step[1] : xe.step[0]);
+                        for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
+                            const int qq = qr < xe.n[0] ? 0 : 1, r = qr - (qq ? xe.n[0] : 0);
+                            const long long zi = zo + (qq ? xe.d[1] : xe.d[0]) + r * (qq ? xe.step[1] : xe.step[0]);
 #pragma unroll
-                        for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = un[v];
+                            for (int v = 0; v < NS; ++v) a.Uout[zi + v * g.cstride] = out[v];
+                        }
                     }
                 }
             }
         }
-#if RING_CTASYNC == 2
-        // Slot release without a CTA-wide barrier: every warp arrives on the slot's "empty"
-        // mbarrier; warp 0 refills whatever slots have been released by all warps (non-blocking
-        // test), and blocks only if the step it needs next has not been issued yet.
-        if (it >= KEEP) {
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
-        }
-        if (tid < 32) {
-            while (next_issue < nsteps) {
-                const int rel = next_issue - D;
-                if (next_issue <= it + 1) mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
-                else if (!mbar_test_warp(&empty[rel % D], (uint32_t)((rel / D) & 1))) break;
-                issue(next_issue);
-                ++next_issue;
-            }
-        }
-#elif RING_CTASYNC
         __syncthreads();
-        if (tid < 32 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
-#else
-        if (it >= KEEP) {
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(&empty[(it - KEEP) % D]);
-        }
-        if (tid < 32) {
-            const int rel = it - KEEP - 1;
-            if (rel >= 0 && rel + D < nsteps) {
-                mbar_wait(&empty[rel % D], (uint32_t)((rel / D) & 1));
-                issue(rel + D);
-            }
-        }
-#endif
+        if (tid == 0 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
     }
 }
 
