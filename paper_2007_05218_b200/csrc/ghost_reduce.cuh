@@ -169,6 +169,39 @@ k_fill_ghost_rows(const __grid_constant__ Geom g, double* __restrict__ U)
 }
 
 // ---- O8 ----------------------------------------------------------------------------
+// Grid-wide max of the per-thread CFL signal `tmax`: warp shuffle, one atomicMax per CTA on the
+// ordered bit pattern; the last CTA to arrive writes dtslot[0] = cfl / max, dtslot[1] = max and
+// resets the workspace.  Called by every thread of every CTA; sm = 8+ words of shared scratch
+// that no thread still reads.  red[0] = running max (as ordered bits), red[1] = CTAs done.
+__device__ __forceinline__ void cfl_reduce_finish(const Geom& g, bool bad, double tmax, unsigned long long* red,
+                                                  double* dtslot, unsigned long long* sm)
+{
+    // t >= 0, so the IEEE bit pattern orders like the value; NaN is mapped above +inf
+    unsigned long long bits = bad ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(tmax);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, bits, o);
+        bits = other > bits ? other : bits;
+    }
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = bits;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int wv = 1; wv < (int)(blockDim.x >> 5); ++wv) bits = sm[wv] > bits ? sm[wv] : bits;
+        atomicMax(red, bits);
+        __threadfence();
+        const unsigned long long nblk = (unsigned long long)gridDim.x * gridDim.y * gridDim.z;
+        if (atomicAdd(red + 1, 1ull) == nblk - 1) {
+            __threadfence();
+            const unsigned long long mx = atomicExch(red, 0ull);   // reset for the next call
+            red[1] = 0ull;
+            const double tm = __longlong_as_double((long long)mx);
+            dtslot[1] = tm;
+            dtslot[0] = g.cfl / tm;
+        }
+    }
+}
+
 // red[0] = running max of t (as ordered bits), red[1] = blocks-done counter,
 // dtslot[0] = dt, dtslot[1] = max t of the last reduction.
 __global__ void __launch_bounds__(256)
@@ -194,31 +227,8 @@ k_estimate_dt(const __grid_constant__ Geom g, const double* __restrict__ U, unsi
         if (!(t == t)) bad = true;
         if (t > tmax) tmax = t;
     }
-    // t >= 0, so the IEEE bit pattern orders like the value; NaN is mapped above +inf
-    unsigned long long bits = bad ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(tmax);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const unsigned long long other = __shfl_xor_sync(0xffffffffu, bits, o);
-        bits = other > bits ? other : bits;
-    }
     __shared__ unsigned long long sm[8];
-    __shared__ bool last;
-    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = bits;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int wv = 1; wv < (int)(blockDim.x >> 5); ++wv) bits = sm[wv] > bits ? sm[wv] : bits;
-        atomicMax(red, bits);
-        __threadfence();
-        last = (atomicAdd(red + 1, 1ull) == gridDim.x - 1);
-        if (last) {
-            __threadfence();
-            const unsigned long long m = atomicExch(red, 0ull);   // reset for the next call
-            red[1] = 0ull;
-            const double tm = __longlong_as_double((long long)m);
-            dtslot[1] = tm;
-            dtslot[0] = g.cfl / tm;
-        }
-    }
+    cfl_reduce_finish(g, bad, tmax, red, dtslot, sm);
 }
 
 // ---- O9 ----------------------------------------------------------------------------

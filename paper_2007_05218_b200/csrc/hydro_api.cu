@@ -50,6 +50,7 @@ struct hydro_ctx {
     int ns_max;
     bool use_ring;            // TMA-ring marching kernels usable for this geometry
     bool split_ghosts;        // hydro_step: x ghost images written by the z sweeps + ghost-row copies
+    bool fuse_dt;             // hydro_step: the stage-1 z hydro sweep also reduces the next step's dt
     CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs on the handle's stream
@@ -277,7 +278,8 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     return HYDRO_OK;
 }
 
-int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev, bool xends = false)
+int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev, bool xends = false,
+                       double *dt_next = nullptr)
 {
     const Geom &g = h->g;
     SweepArgs a;
@@ -290,6 +292,8 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     a.dt = dt;
     a.dt_dev = dt_dev;
     a.xends = (xends && h->use_ring) ? 1 : 0;
+    a.red = (unsigned long long *)(h->scratch + h->cv.red);
+    a.dt_next = (stage == 1 && h->use_ring) ? dt_next : nullptr;
     {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const long long nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
@@ -326,7 +330,11 @@ int fill_ghost_rows_impl(hydro_handle h, int which)
     return check_launch(h, "k_fill_ghost_rows", K_GHOST);
 }
 
-int launch_dt(hydro_handle h)
+// two dt slots of (dt, max t): hydro_step alternates them so that the dt of step s+1, reduced by
+// the last hydro kernel of step s, does not overwrite the dt the rest of step s still reads
+double *dt_slot(hydro_handle h, int slot) { return (double *)(h->scratch + h->cv.dtslot) + 2 * slot; }
+
+int launch_dt(hydro_handle h, int slot = 0)
 {
     const long long nzone = h->g.lcstride * h->g.nboxes;
     long long blocks = (nzone + 255) / 256;
@@ -334,13 +342,13 @@ int launch_dt(hydro_handle h)
     prof_begin(h);
     k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[0],
                                                            (unsigned long long *)(h->scratch + h->cv.red),
-                                                           (double *)(h->scratch + h->cv.dtslot));
+                                                           dt_slot(h, slot));
     return check_launch(h, "k_estimate_dt", K_DT);
 }
 
-int read_dt(hydro_handle h, double *dt_host)
+int read_dt(hydro_handle h, double *dt_host, int slot = 0)
 {
-    cudaError_t e = cudaMemcpyAsync(h->pinned, h->scratch + h->cv.dtslot, 16, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e = cudaMemcpyAsync(h->pinned, dt_slot(h, slot), 16, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("dt read-back: ") + cudaGetErrorString(e));
     const double dt = h->pinned[0], tmax = h->pinned[1];
@@ -402,6 +410,8 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
                 }
     }
     {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
+        const char *ed = getenv("HYDRO_FUSE_DT");
+        h->fuse_dt = h->use_ring && !(ed && atoi(ed) == 0);
         const char *ef = getenv("HYDRO_SPLIT_GHOSTS");
         h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng &&
                           g.nb[2] >= g.ng && !(ef && atoi(ef) == 0);
@@ -470,19 +480,23 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
-    const double *dt_dev = (const double *)(h->scratch + h->cv.dtslot);
     int rc;
-    const bool split = h->split_ghosts;
+    const bool split = h->split_ghosts, fuse = h->fuse_dt;
     for (int s = 0; s < nsteps; ++s) {
-        if ((rc = launch_dt(h))) return rc;
+        const int slot = s & 1;
+        const double *dt_dev = dt_slot(h, slot);
+        // the caller's U0 gets the dt kernel; later steps use the dt that the stage-1 z sweep of the
+        // previous step reduced from the very values it wrote (same formula, same bits)
+        if (s == 0 || !fuse) if ((rc = launch_dt(h, slot))) return rc;
         // the caller's U0 gets the full fill; after that stage 1 has left every valid row of U0
         // complete (x images written by the z sweeps) and only the ghost rows remain
         if ((rc = (split && s > 0) ? fill_ghost_rows_impl(h, 0) : fill_ghosts_impl(h, 0))) return rc;
         if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev, split))) return rc;
         if ((rc = split ? fill_ghost_rows_impl(h, 1) : fill_ghosts_impl(h, 1))) return rc;
-        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split))) return rc;
+        double *dt_next = (fuse && s + 1 < nsteps) ? dt_slot(h, (s + 1) & 1) : nullptr;
+        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split, dt_next))) return rc;
     }
-    if (dt_last_host && nsteps > 0) return read_dt(h, dt_last_host);
+    if (dt_last_host && nsteps > 0) return read_dt(h, dt_last_host, (nsteps - 1) & 1);
     return HYDRO_OK;
 }
 

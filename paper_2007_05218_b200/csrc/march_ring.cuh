@@ -30,6 +30,9 @@
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 
+#define RING_STR2(x) #x
+#define RING_STR(x) RING_STR2(x)
+
 namespace hydro {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
@@ -230,7 +233,14 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 #pragma unroll
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
     const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
+    constexpr bool CFL = FINAL && STAGE == 1;
+    const bool cfl_on = CFL && a.dt_next != nullptr;
+    double tmax = 0.0;
+    bool tbad = false;
 
+#ifdef RING_UNROLL
+_Pragma(RING_STR(unroll RING_UNROLL))
+#endif
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         // early, independent global loads for the update of zone z
@@ -282,6 +292,14 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                     double re = out[4] - K;
                     if (re < g.floor_rhoe) re = g.floor_rhoe;
                     out[5] = re;
+                    if (CFL && cfl_on && m.active) {       // O8 on the zone just formed (same code as k_estimate_dt)
+                        double qn[5], rn;
+                        cons_to_prim(g, out[0], out[1], out[2], out[3], out[5], qn, rn);
+                        const double cs = sqrt(g.gamma * qn[4] * rn);
+                        const double t = (fabs(qn[1]) + cs) * g.dxinv[0] + (fabs(qn[2]) + cs) * g.dxinv[1] + (fabs(qn[3]) + cs) * g.dxinv[2];
+                        if (!(t == t)) tbad = true;
+                        if (t > tmax) tmax = t;
+                    }
                 }
             }
             if (m.active) {          // all stores of the step under one predicate
@@ -317,6 +335,8 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
         __syncthreads();
         if (tid == 0 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
     }
+    if (CFL && cfl_on)
+        cfl_reduce_finish(g, tbad, tmax, a.red, a.dt_next, reinterpret_cast<unsigned long long*>(ring));
 }
 
 // ------------------------------------------------------------------------------------
@@ -375,6 +395,9 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
     double Fnext = 0.0;
 
+#ifdef RING_UNROLL
+_Pragma(RING_STR(unroll RING_UNROLL))
+#endif
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         const double Frho = Fnext;

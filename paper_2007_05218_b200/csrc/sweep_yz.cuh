@@ -28,6 +28,10 @@ struct SweepArgs {
     int seglen;            // zones per pencil segment along DIR
     int sbase;             // first species of this launch (species kernels)
     int xends;             // FINAL ring kernels: also write the x-direction ghost images of every zone
+    // stage-1 FINAL hydro ring kernel: also reduce the CFL signal speed of the state it writes (O8)
+    // and leave the next step's dt in dt_next[0] (max t in dt_next[1]); nullptr = off
+    unsigned long long* red;
+    double* dt_next;
 };
 
 // pencil decode shared by both kernels.  Returns false if the thread has no pencil.
