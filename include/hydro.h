@@ -108,6 +108,15 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
  * NULL) receives the last dt; when it is non-NULL the call synchronises. */
 int hydro_step(hydro_handle h, int nsteps, double *dt_last_host);
 
+/* Which internal paths this handle uses (for bench accounting; they change no result):
+ * what = 0: TMA-ring marching kernels (1) or the plain-load fallback (0);
+ *        1: hydro_step fills ghosts in two parts (x images written by the z sweeps + ghost-row
+ *           copies) instead of one k_fill_ghosts launch per stage;
+ *        2: hydro_step reduces the next step's dt inside the stage-1 z hydro sweep;
+ *        3: passive species per thread and launch in the y/z species sweeps.
+ * Returns -1 for a NULL handle or an unknown `what`. */
+int hydro_query(hydro_handle h, int what);
+
 /* Number of kernel launches this handle has enqueued so far (for bench accounting). */
 long long hydro_launch_count(hydro_handle h);
 

@@ -15,7 +15,7 @@ LIB_PATH = os.environ.get("HYDRO_LIB") or os.path.join(HERE, "libhydro_b200.so")
 HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
-           "hydro_launch_count", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
+           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
 
 
 class HydroParams(C.Structure):
@@ -70,6 +70,7 @@ def lib():
     L.hydro_estimate_dt.argtypes = [vp, dp]
     L.hydro_conserved_totals.argtypes = [vp, C.c_int, dp]
     L.hydro_step.argtypes = [vp, C.c_int, dp]
+    L.hydro_query.argtypes = [vp, C.c_int]
     L.hydro_launch_count.restype = C.c_longlong
     L.hydro_launch_count.argtypes = [vp]
     L.hydro_profile.argtypes = [vp, C.c_int]
@@ -161,6 +162,9 @@ class Hydro:
 
     def hydro_launch_count(self):
         return lib().hydro_launch_count(self.h)
+
+    def hydro_query(self, what):
+        return lib().hydro_query(self.h, what)
 
     KERNEL_CLASSES = ["fill_ghosts", "estimate_dt", "sweep_x", "hydro_y", "species_y", "hydro_z", "species_z",
                       "totals"]

@@ -500,6 +500,18 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
     return HYDRO_OK;
 }
 
+int hydro_query(hydro_handle h, int what)
+{
+    if (!h) return -1;
+    switch (what) {
+        case 0: return h->use_ring ? 1 : 0;
+        case 1: return h->split_ghosts ? 1 : 0;
+        case 2: return h->fuse_dt ? 1 : 0;
+        case 3: return h->ns_max;
+        default: return -1;
+    }
+}
+
 long long hydro_launch_count(hydro_handle h) { return h ? h->launches : 0; }
 
 int hydro_profile(hydro_handle h, int enable)

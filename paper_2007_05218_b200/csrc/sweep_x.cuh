@@ -62,8 +62,10 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     const double* Ub = U + (long long)b * g.bstride + row + ip;
 
     double q[5], rinv;
-    cons_to_prim(g, ldg(Ub), ldg(Ub + g.cstride), ldg(Ub + 2 * g.cstride), ldg(Ub + 3 * g.cstride),
-                 ldg(Ub + 5 * g.cstride), q, rinv);
+    const double* p1 = Ub + g.cstride;
+    const double* p2 = p1 + g.cstride;
+    const double* p3 = p2 + g.cstride;
+    cons_to_prim(g, ldg(Ub), ldg(p1), ldg(p2), ldg(p3), ldg(p3 + 2 * g.cstride), q, rinv);
     double qL[5], qR[5], F[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) ppm_lanes(q[v], qL[v], qR[v]);
@@ -71,45 +73,59 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
 
     const bool store = (lane >= 3) && (lane <= 2 + XW_VALID) && (i < g.nb[0]);
     double* Lb = Lacc + (long long)b * g.lbstride + ((long long)k * g.nb[1] + j) * g.nb[0] + i;
+    {
+        double* pa = Lb;
 #pragma unroll
-    for (int c = 0; c < 5; ++c) {
-        const double Fm = shfl_up1(F[c]);
-        const double acc = -(F[c] - Fm) * g.dxinv[0];
-        if (store) Lb[c * g.lcstride] = acc;
+        for (int c = 0; c < 5; ++c) {
+            const double Fm = shfl_up1(F[c]);
+            const double acc = -(F[c] - Fm) * g.dxinv[0];
+            if (store) *pa = acc;
+            pa += g.lcstride;
+        }
     }
     // species: the loads of group n+1 are issued before group n is reconstructed, so the
     // global-load latency (ncu r01: 40 % of this kernel's stall samples sat on the first use of
     // a species load) is covered by XG species' worth of arithmetic.
     const double Frho = F[0];
-    const double* Us = Ub + 6 * g.cstride;
-    double xc[XG];
+    const double* pl = Ub + 6 * g.cstride;             // next species row to load
+    double* ps = Lb + 5 * g.lcstride;                  // next accumulator row to store
+    int lrem = g.nspec, rem = g.nspec;                 // species not yet loaded / not yet reconstructed
+    auto load = [&](double (&x)[XG]) {
 #pragma unroll
-    for (int q = 0; q < XG; ++q) xc[q] = (q < g.nspec) ? ldg(Us + q * g.cstride) : 0.0;
-    auto species = [&](double raw, int s) {
+        for (int q = 0; q < XG; ++q) { x[q] = (q < lrem) ? ldg(pl) : 0.0; pl += g.cstride; }
+        lrem -= XG;
+    };
+    auto species = [&](double raw) {
         const double X = raw * rinv;
         double XL, XR;
         ppm_lanes(X, XL, XR);
         const double Fs = Frho * (Frho >= 0.0 ? XL : XR);
         const double Fm = shfl_up1(Fs);
         const double acc = -(Fs - Fm) * g.dxinv[0];
-        if (store) Lb[(5 + s) * g.lcstride] = acc;
+        if (store) *ps = acc;
+        ps += g.lcstride;
     };
-    int s0 = 0;
-    for (; s0 + XG <= g.nspec; s0 += XG) {             // full groups: no per-species guard
-        double xn[XG];
+    auto group = [&](const double (&x)[XG]) {
+        if (rem >= XG) {                               // full group: no per-species guard
 #pragma unroll
-        for (int q = 0; q < XG; ++q) {
-            const int s = s0 + XG + q;
-            xn[q] = (s < g.nspec) ? ldg(Us + s * g.cstride) : 0.0;
+            for (int q = 0; q < XG; ++q) species(x[q]);
+        } else {                                       // tail group (warp-uniform guard)
+#pragma unroll
+            for (int q = 0; q < XG - 1; ++q)
+                if (q < rem) species(x[q]);
         }
-#pragma unroll
-        for (int q = 0; q < XG; ++q) species(xc[q], s0 + q);
-#pragma unroll
-        for (int q = 0; q < XG; ++q) xc[q] = xn[q];
+        rem -= XG;
+    };
+    // two register sets alternate (no copies): load one while the other is reconstructed
+    double xa[XG], xb[XG];
+    load(xa);
+    while (rem > 0) {
+        load(xb);
+        group(xa);
+        if (rem <= 0) break;
+        load(xa);
+        group(xb);
     }
-#pragma unroll
-    for (int q = 0; q < XG - 1; ++q)                   // tail group (warp-uniform guard)
-        if (s0 + q < g.nspec) species(xc[q], s0 + q);
 }
 
 }  // namespace hydro

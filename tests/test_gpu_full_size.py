@@ -110,7 +110,14 @@ def test_config5_512cubed_sampled_windows_and_dt():
     dt = h.hydro_estimate_dt()
     assert abs(dt - dt_o) <= 1e-14 * dt_o
     t0 = np.array(h.hydro_conserved_totals(0))
-    dt_step = h.hydro_step(1)                                       # the call bench.py times
+    # the call bench.py times is hydro_step(K): from its second step on, ghosts are filled in two parts
+    # and dt comes out of the z sweep.  Run it for 2 steps on a second handle, and the five separate
+    # calls on this one: step 1 is checked against the oracle below, step 2 must agree bitwise.
+    import torch
+    from paper_2007_05218_b200.binding import Hydro
+    h2 = Hydro(wl.params)
+    h2.U0.copy_(h.U0)
+    dt_step = h.step_explicit()
     assert dt_step == dt
     # windows: inside a box, across a box corner (128-zone boxes), across the periodic domain wrap
     worst = check_windows(wl, h, dt, [(40, 40, 40), (108, 236, 364), (492, 492, 492), (300, 108, 5)])
@@ -118,6 +125,13 @@ def test_config5_512cubed_sampled_windows_and_dt():
     scale = np.abs(t0) + 1e-3                                       # momenta totals are ~0: absolute floor
     assert np.all(np.abs(t1 - t0) <= 1e-13 * np.maximum(scale, 1.0))
     print("config 5 worst window error", worst)
+    dt2 = h.step_explicit()
+    assert h2.hydro_query(1) == 1 and h2.hydro_query(2) == 1        # split ghost fill and fused dt are on
+    assert h2.hydro_step(2) == dt2
+    ng = wl.ng
+    A, B = h.U0.view(wl.state_shape), h2.U0.view(wl.state_shape)
+    for b in range(wl.nboxes):
+        assert torch.equal(A[b, :, ng:-ng, ng:-ng, ng:-ng], B[b, :, ng:-ng, ng:-ng, ng:-ng]), b
 
 
 def test_config4_atmosphere_sampled_windows():
