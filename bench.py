@@ -79,6 +79,23 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
     return out
 
 
+def reduce_max(x, world, device="cpu"):
+    """Max over ranks of a per-rank scalar (the device-timed ms of the timed region): the contract's
+    max-over-ranks rule.  gloo (CPU tensors) in the tests, nccl (device tensors) in the bench."""
+    if world == 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(zones, steps, ms_total, world):
+    """Whole-job zone-updates/s of `world` independent replicas (replicas only)."""
+    return world * zones * steps / (ms_total * 1e-3)
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks / throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -211,12 +228,9 @@ def run_ours(args, rank, world, local_rank):
     launches = h.hydro_launch_count() - launches0
     dt_last = h.hydro_estimate_dt()
     totals = h.hydro_conserved_totals(0)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = reduce_max(ms_total, world, dev)
     ms_step = ms_total / args.steps
-    value = world * wl.zones * args.steps / (ms_total * 1e-3)
+    value = job_value(wl.zones, args.steps, ms_total, world)
 
     # ---- roofline of the dominant kernel class ------------------------------------------
     peak, peak_src = measured_peaks()
@@ -259,17 +273,14 @@ def run_ours(args, rank, world, local_rank):
             B.hydro_run_host(p, host, 1)
         torch.cuda.synchronize(dev)
         el = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([el], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            el = float(t.item())
-        e2e = {"value": world * wl.zones * n_e2e / el, "unit": UNIT, "h2d_bytes_per_step": wl.state_bytes,
+        el = reduce_max(el, world, dev)
+        e2e = {"value": job_value(wl.zones, n_e2e, el * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": wl.state_bytes,
                "d2h_bytes_per_step": wl.state_bytes, "steps": n_e2e, "pinned_host": pinned,
                "api": "hydro_run_host(params, U_host, 1 step)"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu_baseline, _, _ = oracle_sample(1, 0)
+        cpu_baseline, _, _ = oracle_sample(3, 0)      # about 18 s of host work
 
     if rank == 0:
         cfg = workload_config(wl, args.config)

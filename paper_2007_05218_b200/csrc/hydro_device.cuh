@@ -69,10 +69,18 @@ __device__ __forceinline__ void ppm_mono(double el, double er, double a, double&
     const double dm = d * m;
     const bool over_l = dm > t;
     const bool over_r = !over_l && (-t > dm);
+#ifdef PPM_PRED
+    double l1 = el, r1 = er;
+    if (over_l) l1 = 3.0 * a - 2.0 * er;
+    if (over_r) r1 = 3.0 * a - 2.0 * el;
+    if (flat) { l1 = a; r1 = a; }
+    aL = l1; aR = r1;
+#else
     const double l1 = over_l ? 3.0 * a - 2.0 * er : el;
     const double r1 = over_r ? 3.0 * a - 2.0 * el : er;
     aL = flat ? a : l1;
     aR = flat ? a : r1;
+#endif
 }
 
 // ---- division and square root ----------------------------------------------------------

@@ -1,0 +1,51 @@
+"""N > 1 path of bench.py on CPU: two gloo ranks (DESIGN.md sec. 8 -- the hot path does not shard, so
+`--gpus N` is N independent replicas; what the ranks share is the barrier, the max-over-ranks time and
+the whole-job aggregation, and in the reference arm only rank 0 works)."""
+import io
+import os
+import sys
+from contextlib import redirect_stdout
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _rank_main(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    ms_local = 10.0 + 5.0 * rank                       # rank 1 is the slow replica
+    dist.barrier()
+    ms = bench.reduce_max(ms_local, world)
+    value = bench.job_value(1000, 3, ms, world)
+    # reference arm: ranks other than 0 print nothing and do no work
+    out = io.StringIO()
+    if rank != 0:
+        class A:
+            steps, warmup, gpus, config = 1, 0, world, 5
+        with redirect_stdout(out):
+            bench.run_reference(A, rank)
+    q.put((rank, ms, value, out.getvalue()))
+    dist.destroy_process_group()
+
+
+def test_two_rank_aggregation_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_rank_main, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, value, out in res:
+        assert ms == 15.0                               # max over ranks, on every rank
+        assert value == pytest.approx(2 * 1000 * 3 / 0.015)
+        assert out == ""
