@@ -252,12 +252,26 @@ def run_ours(args, rank, world, local_rank):
                                "gbs": step_alg / 1e9 / (ms_step * 1e-3),
                                "frac": step_alg / 1e9 / (ms_step * 1e-3) / peak,
                                "frac_of_nominal_8000": step_alg / 1e9 / (ms_step * 1e-3) / 8000.0}}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")       # written from the committed ncu capture
+    # ncu figures of the committed capture (profiles/traffic.json): DRAM bytes and instruction counts per
+    # launch.  With the live launch durations they give the second roofline: FP64 pipe and issue slots.
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    fp64 = B.hydro_fp64_probe()                               # measured FP64 instr/s of this GPU, now
+    sm_max_hz = (sampler.summary().get("sm_max_mhz") or 1965.0) * 1e6
     if os.path.exists(tr):
         try:
-            roofline["traffic"] = json.load(open(tr)).get(wl.name, {}).get(dom)
+            t = json.load(open(tr)).get(wl.name, {})
+            roofline["traffic"] = t.get("dram_bytes", {}).get(dom)
+            for k, v in kernels.items():
+                wi, fi = t.get("warp_instr", {}).get(k), t.get("fp64_warp_instr", {}).get(k)
+                if wi and fi:
+                    sec = v["ms_per_launch"] * 1e-3
+                    v["fp64_pipe_frac"] = fi * 32 / sec / fp64["dfma"]
+                    v["issue_slot_frac"] = wi / sec / (148 * 4 * sm_max_hz)
         except Exception:
             pass
+    roofline["alu"] = {"fp64_peak_instr_per_s": fp64["dfma"], "fp64_peak_source": "hydro_fp64_probe (independent DFMA chains), this run",
+                       "fp64_pipe_frac": kernels[dom].get("fp64_pipe_frac"), "issue_slot_frac": kernels[dom].get("issue_slot_frac"),
+                       "note": "instruction counts from the committed ncu capture (profiles/traffic.json), durations live"}
 
     # ---- e2e: host buffers through hydro_run_host ---------------------------------------
     del h

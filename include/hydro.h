@@ -136,6 +136,14 @@ int hydro_destroy(hydro_handle h);
  * hydro_init / hydro_run_host on this thread.  Never NULL. */
 const char *hydro_last_error(hydro_handle h);
 
+/* Measurement aid (no part of the path): times three small kernels on the current device and
+ * writes FP64 instructions per second (thread instructions; x2 = FLOP/s for an FMA) into
+ * rates_host[3]: [0] independent DFMA chains, [1] DADD/DMUL chains (no FMA), [2] DFMA chains with
+ * one independent integer multiply-add between consecutive DFMAs (counts the DFMAs only).
+ * Synchronous, default stream, allocates and frees 2.4 MB.  DESIGN.md sec. 5 uses [0] as the
+ * measured FP64 peak. */
+int hydro_fp64_probe(double *rates_host);
+
 /* End-to-end entry for callers without device buffers: U_host (hydro_state_bytes, layout
  * a1, valid zones filled) is copied to the device, advanced nsteps RK2 steps, and copied
  * back in place; dt_host[0..nsteps-1] (may be NULL) receives the timesteps and

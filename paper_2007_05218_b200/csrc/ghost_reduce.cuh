@@ -297,4 +297,31 @@ k_totals_final(const __grid_constant__ Geom g, const double* __restrict__ part, 
     if (threadIdx.x == 0) out[c] = (hi + lo) * g.vol;
 }
 
+// ---- FP64 pipe probe (measurement only: the second roofline of DESIGN.md sec. 5) ----------
+// MODE 0: 8 independent DFMA chains per thread; MODE 1: the same with DADD/DMUL alternating (no
+// FMA); MODE 2: every DFMA followed by one independent integer multiply-add, to see whether the
+// other pipes issue under a busy FP64 pipe or wait for it.  out[] keeps the results alive.
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_fp64_probe(double* out, int iters, double c0, double c1)
+{
+    double x[8];
+    unsigned k[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { x[q] = c0 + (double)(threadIdx.x + q); k[q] = threadIdx.x * 8u + q; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            if (MODE == 1) x[q] = (it & 1) ? __dmul_rn(x[q], c1) : __dadd_rn(x[q], c0);
+            else x[q] = fma(x[q], c1, c0);
+            if (MODE == 2) k[q] = k[q] * 1664525u + (unsigned)it;
+        }
+    }
+    double s = 0.0;
+    unsigned ks = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { s += x[q]; ks += k[q]; }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s + (double)(ks & 1u);
+}
+
 }  // namespace hydro

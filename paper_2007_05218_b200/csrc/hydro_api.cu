@@ -549,6 +549,37 @@ int hydro_destroy(hydro_handle h)
 
 const char *hydro_last_error(hydro_handle h) { return h ? h->err.c_str() : g_init_error.c_str(); }
 
+int hydro_fp64_probe(double *rates_host)
+{
+    if (!rates_host) return fail(nullptr, HYDRO_EINVAL, "null rates_host");
+    const int blocks = 148 * 8, threads = 256, iters = 8192;
+    double *out = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc(&out, (size_t)blocks * threads * 8) != cudaSuccess)
+        return fail(nullptr, HYDRO_ENOMEM, "hydro_fp64_probe: device allocation failed");
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    int rc = HYDRO_OK;
+    for (int mode = 0; mode < 3 && rc == HYDRO_OK; ++mode) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {           // first repetition warms up
+            cudaEventRecord(e0);
+            if (mode == 0) k_fp64_probe<0><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
+            else if (mode == 1) k_fp64_probe<1><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
+            else k_fp64_probe<2><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
+            cudaEventRecord(e1);
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = fail(nullptr, HYDRO_ECUDA, "hydro_fp64_probe: kernel failed"); break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        // FP64 thread-instructions per second (one DFMA = one instruction)
+        rates_host[mode] = (double)blocks * threads * 8.0 * iters / (best * 1e-3);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(out);
+    return rc;
+}
+
 int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt_host, double *totals_host)
 {
     Geom g; std::string why;

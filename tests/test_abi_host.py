@@ -23,7 +23,7 @@ def lib():
 def test_header_symbols_all_exported(lib):
     hdr = open(os.path.join(ROOT, "include", "hydro.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(hydro_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(hydro_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(B.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name

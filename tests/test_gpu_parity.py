@@ -197,6 +197,14 @@ def test_free_stream_and_floor_corner():
     assert np.all(e <= 1e-12), e
 
 
+def test_fp64_probe_is_near_the_derived_peak():
+    from paper_2007_05218_b200 import binding as B
+    r = B.hydro_fp64_probe()
+    derived = 148 * 64 * 1.965e9
+    assert 0.5 * derived < r["dfma"] < 1.1 * derived and 0.5 * derived < r["dadd_dmul"] < 1.1 * derived
+    assert r["dfma_with_imad"] <= 1.02 * r["dfma"]
+
+
 def test_error_codes():
     from paper_2007_05218_b200 import binding as B
     wl = W.uniform((16, 16, 16), (8, 8, 8), 0, (1, 0, 0, 0, 1))
