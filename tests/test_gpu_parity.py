@@ -205,6 +205,58 @@ def test_fp64_probe_is_near_the_derived_peak():
     assert r["dfma_with_imad"] <= 1.02 * r["dfma"]
 
 
+@pytest.mark.parametrize("bcs", [(0, 0, 0), (1, 1, 1), (2, 0, 1)])
+def test_no_write_outside_the_callers_buffers(bcs):
+    """compute-sanitizer is closed on this pool, so out-of-bounds writes are looked for with canaries:
+    U0, U1 and the scratch area are carved out of one allocation with 1 MiB guard bands around each, the
+    whole path (hydro_step with the split ghost fill, totals, the five separate calls) runs, and every
+    guard byte must be untouched.  The states must also come out identical to a run on separate buffers."""
+    import copy
+    import ctypes as C
+    import torch
+    from paper_2007_05218_b200 import binding as B
+    wl = copy.deepcopy(W.config(3, ndom=(64, 16, 24), nbox=(32, 8, 12), nspec=3))
+    wl.params["bc_lo"], wl.params["bc_hi"] = list(bcs), list(bcs)
+    U0 = W.initial_state(wl)
+    p = B.make_params(wl.params)
+    sb, scb = B.hydro_state_bytes(p), B.hydro_scratch_bytes(p)
+    G = 1 << 20
+    up = lambda x: (x + 255) // 256 * 256
+    offs, off = [], G
+    for n in (sb, sb, scb):
+        offs.append(off); off += up(n) + G
+    buf = torch.full((off,), 0xA5, dtype=torch.uint8, device="cuda")
+    base = buf.data_ptr()
+    assert base % 256 == 0
+    u0 = buf[offs[0]:offs[0] + sb].view(torch.float64)
+    u0.copy_(torch.as_tensor(U0).reshape(-1))
+    h = C.c_void_p()
+    L = B.lib()
+    assert L.hydro_init(C.byref(p), base + offs[0], base + offs[1], base + offs[2], scb, None, C.byref(h)) == 0
+    dt = C.c_double()
+    tot = (C.c_double * (5 + wl.nspec))()
+    assert L.hydro_step(h, 3, C.byref(dt)) == 0
+    assert L.hydro_conserved_totals(h, 0, tot) == 0
+    assert L.hydro_estimate_dt(h, C.byref(dt)) == 0
+    for which in (0, 1):
+        assert L.hydro_fill_ghosts(h, which) == 0
+    assert L.hydro_advance_stage(h, 0, dt.value) == 0 and L.hydro_advance_stage(h, 1, dt.value) == 0
+    torch.cuda.synchronize()
+    L.hydro_destroy(h)
+    guard = torch.ones(off, dtype=torch.bool, device="cuda")
+    for o, n in zip(offs, (sb, sb, scb)):
+        guard[o:o + n] = False
+    assert bool((buf[guard] == 0xA5).all())
+    ref = hydro(wl)
+    ref.upload(U0, 0)
+    ref.hydro_step(3)
+    dt2 = ref.hydro_estimate_dt()
+    ref.hydro_fill_ghosts(0); ref.hydro_fill_ghosts(1)
+    ref.hydro_advance_stage(0, dt2); ref.hydro_advance_stage(1, dt2)
+    assert dt2 == dt.value
+    assert torch.equal(ref.U0, u0)
+
+
 def test_error_codes():
     from paper_2007_05218_b200 import binding as B
     wl = W.uniform((16, 16, 16), (8, 8, 8), 0, (1, 0, 0, 0, 1))
