@@ -397,10 +397,11 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     const char *env = getenv("HYDRO_NSMAX");
     h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
-    {   // TMA tensor copies: 16-byte row pitch, row segments that tile the CTA exactly, at most nvar-deep boxes
+    {   // TMA tensor copies: 16-byte row pitch AND 16-byte aligned box starts (the first valid zone of a row sits
+        // ng doubles in, so ng must be even), row segments that tile the CTA exactly
         const int W = g.nb[0] < BS ? g.nb[0] : BS;
         const char *er = getenv("HYDRO_RING");
-        h->use_ring = (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && !(er && atoi(er) == 0);
+        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && !(er && atoi(er) == 0);
         for (int st = 0; st < 2 && h->use_ring; ++st)
             for (int dir = 1; dir <= 2 && h->use_ring; ++dir)
                 for (int nc = 1; nc <= 6 && h->use_ring; ++nc) {

@@ -30,7 +30,16 @@ CASES = {
     "cfg2_sedov_wide_rows": lambda: W.config(2, ndom=(64, 32, 64), nbox=(64, 16, 32), nspec=2),
     "cfg3_ragged_rows": lambda: W.config(3, ndom=(64, 12, 12), nbox=(32, 6, 6)),
     "cfg5_256_wide_box": lambda: W.config(5, ndom=(256, 8, 8), nbox=(256, 8, 8), nspec=4),
+    # ghost widths other than 4: ng = 3 (the minimum the scheme reads), odd ng = 5, wide ng = 6
+    "cfg3_ng3": lambda: with_ng(W.config(3, ndom=(64, 16, 16), nbox=(32, 8, 8), nspec=2), 3),
+    "cfg4_ng5": lambda: with_ng(W.config(4, ndom=(32, 16, 32), nbox=(16, 16, 16), nspec=6), 5),
+    "cfg2_ng6_no_species": lambda: with_ng(W.config(2, ndom=(32, 32, 32), nbox=(32, 16, 16)), 6),
 }
+
+
+def with_ng(wl, ng):
+    wl.params["ng"] = ng
+    return wl
 
 
 @pytest.mark.parametrize("bcs", [(0, 0, 0), (1, 1, 1), (2, 2, 2), (1, 0, 2), (2, 1, 0)])
@@ -75,7 +84,8 @@ def test_one_stage_each_and_dt(name):
 
 
 @pytest.mark.parametrize("name,nsteps", [("cfg1_sod", 20), ("cfg2_sedov_small", 10), ("cfg3_periodic_small", 10),
-                                         ("cfg4_atmosphere_small", 10), ("cfg5_scaling_small", 5)])
+                                         ("cfg4_atmosphere_small", 10), ("cfg5_scaling_small", 5),
+                                         ("cfg3_ng3", 3), ("cfg4_ng5", 3), ("cfg2_ng6_no_species", 3)])
 def test_multi_step(name, nsteps):
     wl = CASES[name]()
     U0 = W.initial_state(wl)
