@@ -15,7 +15,8 @@
 // Measured dead ends (profiles/r01_experiments.md): per-row 1-D bulk copies issued by the 32
 // lanes of warp 0 (ptxas serialises them through ELECT loops: ~10 instructions per copy on the
 // critical warp); per-warp "empty" mbarriers instead of the CTA barrier, blocking or polled;
-// L2 prefetch of the accumulator rows; the accumulator rows through the ring; unroll by 2.
+// L2 prefetch of the accumulator rows; the accumulator rows through the ring; unroll by 2 of
+// the FINAL and species kernels (spills; only the y hydro kernel is unrolled).
 #pragma once
 #include <cuda.h>
 
@@ -30,8 +31,9 @@
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 
-#define RING_STR2(x) #x
-#define RING_STR(x) RING_STR2(x)
+#ifndef RING_UNROLL_Y
+#define RING_UNROLL_Y 2     // unroll of the march loop of the non-FINAL hydro kernel
+#endif
 
 namespace hydro {
 
@@ -238,9 +240,10 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     double tmax = 0.0;
     bool tbad = false;
 
-#ifdef RING_UNROLL
-_Pragma(RING_STR(unroll RING_UNROLL))
-#endif
+    // two steps per trip in the y kernel: the rolling-window rotation becomes register renaming
+    // (8.1 -> 7.6 ms per step at 512^3); the FINAL kernels spill when unrolled and stay at 1
+    constexpr int UNROLL = FINAL ? 1 : RING_UNROLL_Y;
+#pragma unroll UNROLL
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         // early, independent global loads for the update of zone z
@@ -395,9 +398,6 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
     double Fnext = 0.0;
 
-#ifdef RING_UNROLL
-_Pragma(RING_STR(unroll RING_UNROLL))
-#endif
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         const double Frho = Fnext;
