@@ -296,12 +296,11 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     a.dt_next = (stage == 1 && h->use_ring) ? dt_next : nullptr;
     {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
-        const long long nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
-        const long long nw = nchunk * g.nb[1] * g.nb[2] * g.nboxes;
-        const long long blocks = (nw + WARPS - 1) / WARPS;
-        if (blocks > 2147483647LL) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
+        const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
+        const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS);
+        if (gx > 2147483647LL || g.nb[2] > 65535) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
         prof_begin(h);
-        k_sweep_x<WARPS><<<(unsigned)blocks, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc);
+        k_sweep_x<WARPS><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc);
         int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }
