@@ -57,6 +57,8 @@ typedef struct {
     double gamma, cfl;
     double grav[3];
     double small_dens, small_pres;
+    int32_t flatten;            /* 0: off (O1..O9 as in rounds before); 1: shock flattening O10 (needs ng >= 4) */
+    int32_t pad_;
 } oracle_params;
 
 enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2 };
@@ -80,6 +82,7 @@ static int make_geom(const oracle_params *p, geom_t *g)
 {
     if (!p) return -1;
     if (p->ng < 3 || p->nspec < 0) return -1;
+    if (p->flatten != 0 && (p->flatten != 1 || p->ng < 4)) return -1;
     g->nvar = 6 + p->nspec;
     g->nflux = 5 + p->nspec;
     g->nq = 5 + p->nspec;
@@ -271,6 +274,38 @@ void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, in
 /* ---- O2..O7 one RK stage of one box -------------------------------------- */
 /* Us: stage state of this box (ghosts filled), Ubase: U0 of this box (stage 1
  * only), Uout: destination box (valid zones written). */
+/* ---- O10 shock flattening (NEXT-1 of SURVEY 8(f), readings F1..F5) ----
+ * Colella & Woodward 1984 appendix, in the single-pass form used by Castro-type codes, along one
+ * line of n zones with pressure pr[] and the velocity component along the line un[]:
+ *   dp   = pr[i+1] - pr[i-1]
+ *   zeta = |dp| / max(small_pres, |pr[i+2] - pr[i-2]|)
+ *   z    = min(1, max(0, 10*(zeta - 0.75)))                    (ramp from 0.75 to 0.85)
+ *   chi  = (|dp| / min(pr[i+1], pr[i-1]) > 0.33  and  un[i-1] - un[i+1] >= 0) ? 1 : 0
+ *   flat[i] = 1 - max(chi[i]*z[i], chi[i-s]*z[i-s]),  s = +1 if dp[i] > 0 else -1
+ * z, chi are defined for i = 2 .. n-3 and flat for i = 3 .. n-4; other entries are set to 1
+ * (no flattening).  flat = 1 keeps the parabola, flat = 0 replaces it by the zone average. */
+void oracle_flatten_line(const double *pr, const double *un, int n, double small_pres, double *flat)
+{
+    double *zc = (double *)malloc(sizeof(double) * (size_t)n);   /* chi*z */
+    double *dpl = (double *)malloc(sizeof(double) * (size_t)n);
+    for (int i = 0; i < n; ++i) { zc[i] = 0.0; dpl[i] = 0.0; flat[i] = 1.0; }
+    for (int i = 2; i <= n - 3; ++i) {
+        double dp = pr[i + 1] - pr[i - 1];
+        double den = dmax(small_pres, fabs(pr[i + 2] - pr[i - 2]));
+        double zeta = fabs(dp) / den;
+        double z = dmin(1.0, dmax(0.0, 10.0 * (zeta - 0.75)));
+        double chi = 0.0;
+        if (fabs(dp) / dmin(pr[i + 1], pr[i - 1]) > 0.33 && un[i - 1] - un[i + 1] >= 0.0) chi = 1.0;
+        zc[i] = chi * z;
+        dpl[i] = dp;
+    }
+    for (int i = 3; i <= n - 4; ++i) {
+        int sft = dpl[i] > 0.0 ? 1 : -1;
+        flat[i] = 1.0 - dmax(zc[i], zc[i - sft]);
+    }
+    free(dpl); free(zc);
+}
+
 static void advance_box(const oracle_params *p, const geom_t *g, int stage, double dt,
                         const double *Us, const double *Ubase, double *Uout)
 {
@@ -284,6 +319,39 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
         for (int c = 0; c < nvar; ++c) Uc[c] = Us[c * cs + z];
         oracle_cons_to_prim(p->gamma, p->small_dens, p->small_pres, p->nspec, Uc, qz);
         for (int c = 0; c < nq; ++c) q[c * cs + z] = qz[c];
+    }
+    /* O10 (optional): multi-dimensional flattening coefficient = min over the three directions of
+     * the line coefficient, on zones -1 .. nb in every direction (1 elsewhere) */
+    double *flatn = NULL;
+    if (p->flatten) {
+        flatn = (double *)malloc(sizeof(double) * cs);
+        for (size_t z = 0; z < cs; ++z) flatn[z] = 1.0;
+        int nm = 0;
+        for (int d = 0; d < 3; ++d) if (g->nt[d] > nm) nm = g->nt[d];
+        double *pl = (double *)malloc(sizeof(double) * nm);
+        double *ul = (double *)malloc(sizeof(double) * nm);
+        double *fl = (double *)malloc(sizeof(double) * nm);
+        for (int d = 0; d < 3; ++d) {
+            const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+            for (int t2 = ng - 1; t2 <= ng + g->nb[d2]; ++t2)
+            for (int t1 = ng - 1; t1 <= ng + g->nb[d1]; ++t1) {
+                int ijk[3];
+                ijk[d1] = t1; ijk[d2] = t2;
+                for (int m = 0; m < g->nt[d]; ++m) {
+                    ijk[d] = m;
+                    size_t z = zidx(g, ijk[0], ijk[1], ijk[2]);
+                    pl[m] = q[4 * cs + z];
+                    ul[m] = q[(1 + d) * cs + z];
+                }
+                oracle_flatten_line(pl, ul, g->nt[d], p->small_pres, fl);
+                for (int m = ng - 1; m <= ng + g->nb[d]; ++m) {
+                    ijk[d] = m;
+                    size_t z = zidx(g, ijk[0], ijk[1], ijk[2]);
+                    flatn[z] = dmin(flatn[z], fl[m]);
+                }
+            }
+        }
+        free(fl); free(ul); free(pl);
     }
     /* O3-O5: face fluxes per direction.  F[d] holds NFLUX x (faces of d),
      * face (i,j,k) of direction d = low face of valid zone (i,j,k), with the
@@ -319,6 +387,15 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
                     line[c * nmax + m] = q[c * cs + zidx(g, ijk[0], ijk[1], ijk[2])];
                 }
                 oracle_ppm_line(line + c * nmax, n, sl, ed, lL + c * nmax, lR + c * nmax);
+                if (flatn) {   /* O10: blend the monotonised parabola with the zone average */
+                    for (int m = 2; m <= n - 3; ++m) {
+                        ijk[d] = m - 3 + ng;
+                        const double f = flatn[zidx(g, ijk[0], ijk[1], ijk[2])];
+                        const double omf = 1.0 - f;
+                        lL[c * nmax + m] = f * lL[c * nmax + m] + omf * line[c * nmax + m];
+                        lR[c * nmax + m] = f * lR[c * nmax + m] + omf * line[c * nmax + m];
+                    }
+                }
             }
             /* face f (0..nb[d]) lies between line zones m = f+2 and m = f+3 */
             for (int f = 0; f <= g->nb[d]; ++f) {
@@ -379,6 +456,7 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
     free(L);
     free(Ff); free(fR); free(fL); free(lR); free(lL); free(ed); free(sl); free(line);
     for (int d = 0; d < 3; ++d) free(F[d]);
+    free(flatn);
     free(qz); free(Uc); free(q);
 }
 

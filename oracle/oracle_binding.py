@@ -18,6 +18,7 @@ class OracleParams(C.Structure):
         ("prob_lo", C.c_double * 3), ("prob_hi", C.c_double * 3),
         ("gamma", C.c_double), ("cfl", C.c_double), ("grav", C.c_double * 3),
         ("small_dens", C.c_double), ("small_pres", C.c_double),
+        ("flatten", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -31,6 +32,7 @@ def make_params(d: dict) -> OracleParams:
     p.ng, p.nspec = int(d["ng"]), int(d["nspec"])
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
+    p.flatten = int(d.get("flatten", 0))
     return p
 
 
@@ -55,6 +57,8 @@ def lib():
         L.oracle_cons_to_prim.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, dp, dp]
         L.oracle_ppm_line.restype = None
         L.oracle_ppm_line.argtypes = [dp, C.c_int, dp, dp, dp, dp]
+        L.oracle_flatten_line.restype = None
+        L.oracle_flatten_line.argtypes = [dp, dp, C.c_int, C.c_double, dp]
         L.oracle_hllc.restype = None
         L.oracle_hllc.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp]
         L.oracle_max_threads.restype = C.c_int
@@ -124,6 +128,14 @@ def ppm_line(a):
     s, e, aL, aR = (np.zeros(n) for _ in range(4))
     lib().oracle_ppm_line(_ptr(a), n, _ptr(s), _ptr(e), _ptr(aL), _ptr(aR))
     return s, e, aL, aR
+
+
+def flatten_line(pr, un, small_pres=1e-14):
+    pr = np.ascontiguousarray(pr, dtype=np.float64)
+    un = np.ascontiguousarray(un, dtype=np.float64)
+    flat = np.zeros(pr.size)
+    lib().oracle_flatten_line(_ptr(pr), _ptr(un), pr.size, small_pres, _ptr(flat))
+    return flat
 
 
 def hllc(direction, gamma, qL, qR, small_dens=1e-12, small_pres=1e-14):

@@ -38,6 +38,8 @@ def make_params(d: dict) -> HydroParams:
     p.ng, p.nspec = int(d["ng"]), int(d["nspec"])
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
+    if int(d.get("flatten", 0)) != 0:
+        raise NotImplementedError("shock flattening (O10) exists in the oracle only so far")
     return p
 
 
