@@ -60,6 +60,8 @@ typedef struct {
     double  gamma, cfl;
     double  grav[3];            /* constant acceleration; {0,0,0} disables the source        */
     double  small_dens, small_pres; /* floors (1e-12, 1e-14 in all workloads)                */
+    int32_t flatten;            /* 0: off; 1: PPM shock flattening O10, needs ng >= 4 */
+    int32_t reserved_;          /* keep 0 */
 } hydro_params;
 
 typedef struct hydro_ctx *hydro_handle;
@@ -123,10 +125,10 @@ long long hydro_launch_count(hydro_handle h);
 /* Optional per-launch timing for measurement (bench.py's roofline object).  While enabled,
  * every kernel launch of this handle is bracketed by a CUDA event pair on the handle's stream.
  * hydro_profile_read synchronises, then writes the summed device time in ms and the launch
- * count of each kernel class into ms_host[8] / count_host[8] and clears the record.
+ * count of each kernel class into ms_host[HYDRO_NCLASS] / count_host[HYDRO_NCLASS] and clears the record.
  * Classes: 0 ghost fill, 1 dt reduction, 2 x sweep, 3 y hydro sweep, 4 y species sweep,
- * 5 z hydro sweep + update, 6 z species sweep + update, 7 totals. */
-#define HYDRO_NCLASS 8
+ * 5 z hydro sweep + update, 6 z species sweep + update, 7 totals, 8 flattening coefficients. */
+#define HYDRO_NCLASS 9
 int hydro_profile(hydro_handle h, int enable);
 int hydro_profile_read(hydro_handle h, double *ms_host, long long *count_host);
 

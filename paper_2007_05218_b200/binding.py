@@ -26,6 +26,7 @@ class HydroParams(C.Structure):
         ("prob_lo", C.c_double * 3), ("prob_hi", C.c_double * 3),
         ("gamma", C.c_double), ("cfl", C.c_double), ("grav", C.c_double * 3),
         ("small_dens", C.c_double), ("small_pres", C.c_double),
+        ("flatten", C.c_int32), ("reserved_", C.c_int32),
     ]
 
 
@@ -38,8 +39,7 @@ def make_params(d: dict) -> HydroParams:
     p.ng, p.nspec = int(d["ng"]), int(d["nspec"])
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
-    if int(d.get("flatten", 0)) != 0:
-        raise NotImplementedError("shock flattening (O10) exists in the oracle only so far")
+    p.flatten = int(d.get("flatten", 0))
     return p
 
 
@@ -179,14 +179,14 @@ class Hydro:
         return lib().hydro_query(self.h, what)
 
     KERNEL_CLASSES = ["fill_ghosts", "estimate_dt", "sweep_x", "hydro_y", "species_y", "hydro_z", "species_z",
-                      "totals"]
+                      "totals", "flatten"]
 
     def hydro_profile(self, enable):
         self._check(lib().hydro_profile(self.h, int(enable)))
 
     def hydro_profile_read(self):
-        ms = (C.c_double * 8)()
-        cnt = (C.c_longlong * 8)()
+        ms = (C.c_double * 9)()
+        cnt = (C.c_longlong * 9)()
         self._check(lib().hydro_profile_read(self.h, ms, cnt))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_CLASSES)}
 

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhydro_b200.so")
 SOURCES = ["hydro_api.cu"]
-HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_yz.cuh", "march_ring.cuh", "ghost_reduce.cuh"]
+HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_yz.cuh", "march_ring.cuh", "ghost_reduce.cuh", "flatten.cuh"]
 
 
 def nvcc_cmd(fmad: bool, out: str = LIB, extra=()):

@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "ghost_reduce.cuh"
+#include "flatten.cuh"
 #include "hydro_device.cuh"
 #include "sweep_x.cuh"
 #include "sweep_yz.cuh"
@@ -32,7 +33,7 @@ constexpr int RING_D = HYDRO_RING_D;  // depth of the TMA ring of the marching k
 thread_local std::string g_init_error = "";
 
 struct Carve {
-    size_t lacc, frho, part, totals, red, dtslot, total;
+    size_t lacc, frho, part, totals, red, dtslot, flat, total;
 };
 
 }  // namespace
@@ -52,6 +53,7 @@ struct hydro_ctx {
     bool split_ghosts;        // hydro_step: x ghost images written by the z sweeps + ghost-row copies
     bool fuse_dt;             // hydro_step: the stage-1 z hydro sweep also reduces the next step's dt
     CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
+    CUtensorMap fmaps[2];      // [DIR-1]: TMA views of the flattening-coefficient array (flatten == 1)
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs on the handle's stream
     bool profiling;
@@ -68,7 +70,10 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
     if (p->ng < 3) { why = "ng must be >= 3"; return false; }
     if (p->nspec < 0) { why = "nspec must be >= 0"; return false; }
     if (!(p->gamma > 1.0)) { why = "gamma must be > 1"; return false; }
+    if (p->flatten != 0 && p->flatten != 1) { why = "flatten must be 0 or 1"; return false; }
+    if (p->flatten == 1 && p->ng < 4) { why = "flattening needs ng >= 4"; return false; }
     std::memset(&g, 0, sizeof(g));
+    g.flatten = p->flatten;
     g.ng = p->ng; g.nspec = p->nspec; g.nvar = 6 + p->nspec; g.nflux = 5 + p->nspec;
     g.nboxes = 1;
     double dx[3];
@@ -121,6 +126,7 @@ Carve carve(const Geom &g)
     c.totals = off; off += up256((size_t)g.nflux * 8);
     c.red = off;    off += 256;
     c.dtslot = off; off += 256;
+    c.flat = off;   if (g.flatten) off += up256((size_t)g.cstride * g.nboxes * 8);   // O10 coefficients
     c.total = off;
     return c;
 }
@@ -128,8 +134,11 @@ Carve carve(const Geom &g)
 // TMA view of one state for the ring kernels of direction dir (1: y march, 2: z march): a 5-D
 // tensor (i, j, k, component, box) with a box of W zones x R rows x nc components, R counted
 // along the transverse dimension (k for the y march, j for the z march).
-bool make_ring_map(CUtensorMap *out, double *U, const Geom &g, int dir, int nc, std::string &why)
+bool make_ring_map(CUtensorMap *out, double *U, const Geom &g, int dir, int nc, std::string &why,
+                   int ncomp_total = -1, long long box_stride = -1)
 {
+    if (ncomp_total < 0) ncomp_total = g.nvar;
+    if (box_stride < 0) box_stride = g.bstride;
     typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -144,10 +153,10 @@ bool make_ring_map(CUtensorMap *out, double *U, const Geom &g, int dir, int nc, 
         encode = (encode_fn)fn;
     }
     const int W = g.nb[0] < BS ? g.nb[0] : BS, R = BS / W;
-    cuuint64_t dims[5] = {(cuuint64_t)g.nt[0], (cuuint64_t)g.nt[1], (cuuint64_t)g.nt[2], (cuuint64_t)g.nvar,
+    cuuint64_t dims[5] = {(cuuint64_t)g.nt[0], (cuuint64_t)g.nt[1], (cuuint64_t)g.nt[2], (cuuint64_t)ncomp_total,
                           (cuuint64_t)g.nboxes};
     cuuint64_t strides[4] = {(cuuint64_t)g.nt[0] * 8, (cuuint64_t)g.nt[0] * g.nt[1] * 8, (cuuint64_t)g.cstride * 8,
-                             (cuuint64_t)g.bstride * 8};
+                             (cuuint64_t)box_stride * 8};
     cuuint32_t box[5] = {(cuuint32_t)W, dir == 2 ? (cuuint32_t)R : 1u, dir == 1 ? (cuuint32_t)R : 1u, (cuuint32_t)nc, 1u};
     cuuint32_t estr[5] = {1, 1, 1, 1, 1};
     CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -163,7 +172,7 @@ int fail(hydro_handle h, int code, const std::string &msg)
 }
 
 // kernel classes of hydro_profile_read
-enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIES_Z, K_TOTALS, K_NCLASS };
+enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIES_Z, K_TOTALS, K_FLATTEN, K_NCLASS };
 
 void prof_begin(hydro_handle h)
 {
@@ -205,22 +214,46 @@ void set_smem(K kernel, size_t bytes)
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+template <int DIR, bool FINAL, int STAGE, int N, bool FLAT>
+void launch_species_ring_n(hydro_handle h, const SweepArgs &a, dim3 grid, const RingMaps &tm)
+{
+    const size_t sm = (size_t)RING_D * (1 + N + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
+    auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D, FLAT>;
+    static bool once = (set_smem(kern, sm), true); (void)once;
+    kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
+}
+
 template <int DIR, bool FINAL, int STAGE>
 void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, int state)
 {
     RingMaps tm;
     tm.a = h->maps[state][DIR - 1][1];
     tm.b = h->maps[state][DIR - 1][ns];
+    tm.f = h->fmaps[DIR - 1];
+    const bool flat = h->g.flatten != 0;
     switch (ns) {
-#define CASE(N) case N: { \
-        const size_t sm = (size_t)RING_D * (1 + N) * BS * 8 + RING_D * 8; \
-        auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D>; \
-        static bool once = (set_smem(kern, sm), true); (void)once; \
-        kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } break;
+#define CASE(N) case N: \
+        if (flat) launch_species_ring_n<DIR, FINAL, STAGE, N, true>(h, a, grid, tm); \
+        else launch_species_ring_n<DIR, FINAL, STAGE, N, false>(h, a, grid, tm); \
+        break;
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
         default: break;
     }
+}
+
+template <int DIR, bool FINAL, int STAGE, bool FLAT>
+void launch_hydro_ring(hydro_handle h, const SweepArgs &a, dim3 grid, int state)
+{
+    constexpr int NROW = (FINAL ? 6 : 5) + (FLAT ? 1 : 0);
+    const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
+    auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D, FLAT>;
+    static bool once = (set_smem(kern, sm), true); (void)once;
+    RingMaps tm;
+    tm.a = h->maps[state][DIR - 1][FINAL ? 6 : 4];
+    tm.b = h->maps[state][DIR - 1][1];
+    tm.f = h->fmaps[DIR - 1];
+    kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
 
 template <int DIR, bool FINAL, int STAGE>
@@ -249,14 +282,8 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     }
     prof_begin(h);
     if (ring) {
-        constexpr int NROW = FINAL ? 6 : 5;
-        const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
-        auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D>;
-        static bool once = (set_smem(kern, sm), true); (void)once;
-        RingMaps tm;
-        tm.a = h->maps[state][DIR - 1][FINAL ? 6 : 4];
-        tm.b = h->maps[state][DIR - 1][1];
-        kern<<<grid, BS, sm, h->stream>>>(g, a, tm);
+        if (g.flatten) launch_hydro_ring<DIR, FINAL, STAGE, true>(h, a, grid, state);
+        else launch_hydro_ring<DIR, FINAL, STAGE, false>(h, a, grid, state);
     } else
         k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
@@ -294,13 +321,26 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     a.xends = (xends && h->use_ring) ? 1 : 0;
     a.red = (unsigned long long *)(h->scratch + h->cv.red);
     a.dt_next = (stage == 1 && h->use_ring) ? dt_next : nullptr;
+    a.FL = nullptr;
+    if (g.flatten) {   // O10: flattening coefficients of the stage state (ghosts are filled) before any sweep
+        a.FL = (const double *)(h->scratch + h->cv.flat);
+        const int xblocks = (g.nb[0] + 2 + 127) / 128;
+        prof_begin(h);
+        k_flatten<<<dim3(xblocks * (g.nb[1] + 2), g.nb[2] + 2, g.nboxes), 128, 0, h->stream>>>(
+            g, a.Us, (double *)(h->scratch + h->cv.flat));
+        int rc = check_launch(h, "k_flatten", K_FLATTEN);
+        if (rc) return rc;
+    }
     {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
         const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS);
         if (gx > 2147483647LL || g.nb[2] > 65535) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
         prof_begin(h);
-        k_sweep_x<WARPS><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc);
+        if (g.flatten)
+            k_sweep_x<WARPS, true><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
+        else
+            k_sweep_x<WARPS, false><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
         int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }
@@ -408,6 +448,14 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
                     std::string why2;
                     if (!make_ring_map(&h->maps[st][dir - 1][nc], h->U[st], g, dir, nc, why2)) h->use_ring = false;
                 }
+    }
+    if (g.flatten) {   // coefficient array = 1 (no flattening) outside the zones k_flatten writes
+        double *FL = (double *)(h->scratch + cv.flat);
+        k_fill_value<<<148 * 8, 256, 0, h->stream>>>(FL, (long long)g.cstride * g.nboxes, 1.0);
+        for (int dir = 1; dir <= 2 && h->use_ring; ++dir) {
+            std::string why2;
+            if (!make_ring_map(&h->fmaps[dir - 1], FL, g, dir, 1, why2, 1, g.cstride)) h->use_ring = false;
+        }
     }
     {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
         const char *ed = getenv("HYDRO_FUSE_DT");

@@ -23,7 +23,7 @@ struct Geom {
     int NB[3];       // boxes per dimension
     int ndom[3];
     int bc_lo[3], bc_hi[3];
-    int ng, nspec, nvar, nflux, nboxes, has_grav;
+    int ng, nspec, nvar, nflux, nboxes, has_grav, flatten;
     long long cstride;   // doubles per (box, component) of a state     = nt0*nt1*nt2
     long long bstride;   // doubles per box of a state                  = cstride*nvar
     long long lcstride;  // doubles per (box, component) of the accumulator = nb0*nb1*nb2

@@ -23,6 +23,7 @@
 #include "hydro_device.cuh"
 #include "sweep_yz.cuh"
 #include "ghost_reduce.cuh"
+#include "flatten.cuh"
 
 #ifndef RING_MINB
 #define RING_MINB 3        // CTAs per SM the hydro kernels' register allocation is capped for
@@ -85,6 +86,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 // stage state with boxes {W, R rows, NCa components} and {W, R rows, NCb components}.
 struct RingMaps {
     CUtensorMap a, b;
+    CUtensorMap f;       // flattening coefficients (FLAT kernels): {W, R rows, 1} boxes of the FL array
 };
 
 // Decomposition of a CTA into R row segments of W zones.
@@ -183,11 +185,12 @@ __device__ __forceinline__ XEnds xends_setup(const Geom& g, bool on, int b, int 
 // ------------------------------------------------------------------------------------
 // hydro variables.  Ring rows: non-FINAL  rho, mx, my, mz (map a, 4 components) + rho*e (map b,
 // 1 component); FINAL  rho, mx, my, mz, rho*E, rho*e (map a, 6 components).
-template <int DIR, bool FINAL, int STAGE, int BS, int D>
+template <int DIR, bool FINAL, int STAGE, int BS, int D, bool FLAT>
 __global__ void __launch_bounds__(BS, RING_MINB)
 k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
-    constexpr int NROW = FINAL ? 6 : 5;
+    constexpr int ROW_F = FINAL ? 6 : 5;      // ring row of the flattening coefficient (FLAT)
+    constexpr int NROW = ROW_F + (FLAT ? 1 : 0);
     constexpr int KEEP = FINAL ? 3 : 0;
     constexpr int ROW_E = FINAL ? 5 : 4;       // ring row of rho*e
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -212,11 +215,13 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
             ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
             ring_issue<DIR>(g, m, &tm.b, slot + 4 * BS, bar, m0 - 3 + it, 5, b);
         }
+        if (FLAT) ring_issue<DIR>(g, m, &tm.f, slot + ROW_F * BS, bar, m0 - 3 + it, 0, b);
     };
 
     if (tid == 0) {
         tma_prefetch_desc(&tm.a);
         if (!FINAL) tma_prefetch_desc(&tm.b);
+        if (FLAT) tma_prefetch_desc(&tm.f);
         for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
@@ -235,6 +240,7 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 #pragma unroll
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
     const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
+    double f1 = 1.0, f2 = 1.0;               // O10 coefficients of zones n-1, n-2 (FLAT)
     constexpr bool CFL = FINAL && STAGE == 1;
     const bool cfl_on = CFL && a.dt_next != nullptr;
     double tmax = 0.0;
@@ -260,6 +266,8 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         double q[5], rinv;
         cons_to_prim(g, slot[tid], slot[BS + tid], slot[2 * BS + tid], slot[3 * BS + tid], slot[ROW_E * BS + tid], q, rinv);
+        const double fn = FLAT ? slot[ROW_F * BS + tid] : 1.0;   // O10 coefficient of the new zone
+        const double omf2 = 1.0 - f2;
         double qL[5], qR[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -267,10 +275,12 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
             const double en = ppm_edge(a2[v], a1[v], s1[v], sn);
             double aL, aR;
             ppm_mono(e1[v], en, a2[v], aL, aR);
+            if (FLAT) flat_blend(f2, omf2, a2[v], aL, aR);
             qL[v] = aR1[v];
             qR[v] = aL;
             a2[v] = a1[v]; a1[v] = q[v]; s1[v] = sn; e1[v] = en; aR1[v] = aR;
         }
+        f2 = f1; f1 = fn;
         if (it >= 5) {
             double F[5];
             hllc<DIR>(g, qL, qR, F);
@@ -345,11 +355,12 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 // ------------------------------------------------------------------------------------
 // NS passive species per thread.  Ring rows: rho (map a, 1 component) + rho*X_k, k = sbase..
 // sbase+NS-1 (map b, NS components).
-template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D>
+template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT>
 __global__ void __launch_bounds__(BS, RING_MINB_S)
 k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
-    constexpr int NROW = 1 + NS;
+    constexpr int ROW_F = 1 + NS;             // ring row of the flattening coefficient (FLAT)
+    constexpr int NROW = ROW_F + (FLAT ? 1 : 0);
     constexpr int KEEP = FINAL ? 3 : 0;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
@@ -371,11 +382,13 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
         ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
         ring_issue<DIR>(g, m, &tm.b, slot + BS, bar, m0 - 3 + it, 6 + sbase, b);
+        if (FLAT) ring_issue<DIR>(g, m, &tm.f, slot + ROW_F * BS, bar, m0 - 3 + it, 0, b);
     };
 
     if (tid == 0) {
         tma_prefetch_desc(&tm.a);
         tma_prefetch_desc(&tm.b);
+        if (FLAT) tma_prefetch_desc(&tm.f);
         for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
@@ -397,6 +410,7 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     // F_rho of the face handled at step `it` is loaded one step ahead (ncu r01: 23-25 % of this
     // kernel's stall samples sat on its first use when it was loaded at the top of its own step)
     double Fnext = 0.0;
+    double f1 = 1.0, f2 = 1.0;               // O10 coefficients of zones n-1, n-2 (FLAT)
 
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
@@ -414,6 +428,8 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
         const double rinv = drcp(dmax(slot[tid], g.small_dens));
+        const double fn = FLAT ? slot[ROW_F * BS + tid] : 1.0;
+        const double omf2 = 1.0 - f2;
         // pass 1: reconstruction and face fluxes of all NS species (no global operand)
         double out[NS];
 #pragma unroll
@@ -423,11 +439,13 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
             const double en = ppm_edge(a2[v], a1[v], s1[v], sn);
             double aL, aR;
             ppm_mono(e1[v], en, a2[v], aL, aR);
+            if (FLAT) flat_blend(f2, omf2, a2[v], aL, aR);
             const double Fs = Frho * (Frho >= 0.0 ? aR1[v] : aL);
             a2[v] = a1[v]; a1[v] = X; s1[v] = sn; e1[v] = en; aR1[v] = aR;
             out[v] = Fs - Fp[v];
             Fp[v] = Fs;
         }
+        f2 = f1; f1 = fn;
         // pass 2: accumulator / stage update (first use of this step's global loads)
         if (upd) {
 #pragma unroll

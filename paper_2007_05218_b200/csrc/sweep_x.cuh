@@ -12,6 +12,7 @@
 // face mass-flux array is needed in x).
 #pragma once
 #include "hydro_device.cuh"
+#include "flatten.cuh"
 
 namespace hydro {
 
@@ -27,7 +28,8 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(F
 
 // PPM along the lanes: returns the face states of face i+1/2 (between this lane's zone
 // and the next lane's): qLf = aR(i), qRf = aL(i+1).  Valid for lanes 2..28.
-__device__ __forceinline__ void ppm_lanes(double a, double& qLf, double& qRf)
+template <bool FLAT>
+__device__ __forceinline__ void ppm_lanes(double a, double f, double omf, double& qLf, double& qRf)
 {
     const double ap = shfl_dn1(a), am = shfl_up1(a);
     const double s = ppm_slope(am, a, ap);             // lanes 1..30
@@ -36,13 +38,15 @@ __device__ __forceinline__ void ppm_lanes(double a, double& qLf, double& qRf)
     const double em = shfl_up1(e);                     // e_{i-1/2}, lanes 2..30
     double aL, aR;
     ppm_mono(em, e, a, aL, aR);                        // lanes 2..29
+    if (FLAT) flat_blend(f, omf, a, aL, aR);           // O10 (this lane's zone)
     qLf = aR;
     qRf = shfl_dn1(aL);                                // lanes 2..28
 }
 
-template <int WARPS>
+template <int WARPS, bool FLAT>
 __global__ void __launch_bounds__(WARPS * 32)
-k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ Lacc)
+k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ Lacc,
+          const double* __restrict__ FL)
 {
     const int lane = threadIdx.x & 31;
     const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
@@ -62,6 +66,8 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     const long long row = ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0];
     const double* Ub = U + (long long)b * g.bstride + row + ip;
 
+    double fl = 1.0, omf = 0.0;
+    if (FLAT) { fl = ldg(FL + (long long)b * g.cstride + row + ip); omf = 1.0 - fl; }
     double q[5], rinv;
     const double* p1 = Ub + g.cstride;
     const double* p2 = p1 + g.cstride;
@@ -69,7 +75,7 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     cons_to_prim(g, ldg(Ub), ldg(p1), ldg(p2), ldg(p3), ldg(p3 + 2 * g.cstride), q, rinv);
     double qL[5], qR[5], F[5];
 #pragma unroll
-    for (int v = 0; v < 5; ++v) ppm_lanes(q[v], qL[v], qR[v]);
+    for (int v = 0; v < 5; ++v) ppm_lanes<FLAT>(q[v], fl, omf, qL[v], qR[v]);
     hllc<0>(g, qL, qR, F);                             // face i+1/2, lanes 2..28
 
     const bool store = (lane >= 3) && (lane <= 2 + XW_VALID) && (i < g.nb[0]);
@@ -99,7 +105,7 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     auto species = [&](double raw) {
         const double X = raw * rinv;
         double XL, XR;
-        ppm_lanes(X, XL, XR);
+        ppm_lanes<FLAT>(X, fl, omf, XL, XR);
         const double Fs = Frho * (Frho >= 0.0 ? XL : XR);
         const double Fm = shfl_up1(Fs);
         const double acc = -(Fs - Fm) * g.dxinv[0];

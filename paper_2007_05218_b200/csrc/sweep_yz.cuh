@@ -14,6 +14,7 @@
 // L = -(dFx)*dxinv - (dFy)*dyinv - (dFz)*dzinv in exactly that association (O6).
 #pragma once
 #include "hydro_device.cuh"
+#include "flatten.cuh"
 
 namespace hydro {
 
@@ -32,6 +33,7 @@ struct SweepArgs {
     // and leave the next step's dt in dt_next[0] (max t in dt_next[1]); nullptr = off
     unsigned long long* red;
     double* dt_next;
+    const double* FL;      // O10 flattening coefficients (padded, one array per box) or nullptr
 };
 
 // pencil decode shared by both kernels.  Returns false if the thread has no pencil.
@@ -84,6 +86,10 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
         cons_to_prim(g, ldg(Un), ldg(Un + g.cstride), ldg(Un + 2 * g.cstride), ldg(Un + 3 * g.cstride),
                      ldg(Un + 5 * g.cstride), q, rinv);
         double qL[5], qR[5];
+        // O10 coefficient of zone n-2 (defined on zones -1 .. nb; the other parabolas are not used)
+        const bool flat = a.FL != nullptr && n - 2 >= -1 && n - 2 <= g.nb[DIR];
+        const double f2 = flat ? ldg(a.FL + (long long)b * g.cstride + z0 + (long long)(n - 2) * mstride) : 1.0;
+        const double omf2 = 1.0 - f2;
         // window before the shift: a1 = a[n-1], a2 = a[n-2], s1 = s[n-2], e1 = e[n-5/2], aR1 = aR(n-3)
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
@@ -91,6 +97,7 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
             const double en = ppm_edge(a2[v], a1[v], s1[v], sn);    // e[n-3/2]   (n >= m0)
             double aL, aR;
             ppm_mono(e1[v], en, a2[v], aL, aR);                     // zone n-2   (n >= m0+1)
+            if (flat) flat_blend(f2, omf2, a2[v], aL, aR);
             qL[v] = aR1[v];                                         // face n-5/2 (n >= m0+2)
             qR[v] = aL;
             a2[v] = a1[v]; a1[v] = q[v]; s1[v] = sn; e1[v] = en; aR1[v] = aR;
@@ -172,6 +179,9 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         const double Frho = haveF ? ldg(Fb + (long long)(n - 2) * fmstride) : 0.0;
         const bool upd = (n >= m0 + 3);
         const int z = n - 3;
+        const bool flat = a.FL != nullptr && n - 2 >= -1 && n - 2 <= g.nb[DIR];
+        const double f2 = flat ? ldg(a.FL + (long long)b * g.cstride + z0 + (long long)(n - 2) * mstride) : 1.0;
+        const double omf2 = 1.0 - f2;
 #pragma unroll
         for (int v = 0; v < NS; ++v) {
             const double X = ldg(Xb + n * mstride + v * g.cstride) * rinv;
@@ -179,6 +189,7 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
             const double en = ppm_edge(a2[v], a1[v], s1[v], sn);
             double aL, aR;
             ppm_mono(e1[v], en, a2[v], aL, aR);
+            if (flat) flat_blend(f2, omf2, a2[v], aL, aR);
             const double Fs = Frho * (Frho >= 0.0 ? aR1[v] : aL);
             a2[v] = a1[v]; a1[v] = X; s1[v] = sn; e1[v] = en; aR1[v] = aR;
             if (upd) {

@@ -105,6 +105,64 @@ def test_multi_step(name, nsteps):
     assert np.all(np.abs(tg - to) <= 1e-10 * scale)
 
 
+# ---- O10 shock flattening (optional) ---------------------------------------------
+FLAT_CASES = ["cfg1_sod", "cfg2_sedov_small", "cfg4_atmosphere_small", "cfg5_scaling_small",
+              "cfg3_one_species_odd_box", "cfg2_sedov_wide_rows", "cfg2_ng6_no_species"]
+
+
+def flat_case(name):
+    wl = CASES[name]()
+    wl.params["flatten"] = 1
+    return wl
+
+
+@pytest.mark.parametrize("name", FLAT_CASES)
+def test_flatten_one_step_and_three_steps(name):
+    wl = flat_case(name)
+    U0 = W.initial_state(wl, ghost_value=np.nan)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.step_explicit()
+    assert abs(dt_g - dt_o) <= 1e-14 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-12), e
+    for s in range(2):
+        dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.hydro_step(2)                       # split ghost fill + fused dt with flattening on
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-11), e
+
+
+def test_flatten_changes_shocks_and_is_a_bitwise_noop_without_them():
+    # Sod: the flattened run differs from the plain one (the coefficient is active) ...
+    wl0, wl1 = CASES["cfg1_sod"](), flat_case("cfg1_sod")
+    U0 = W.initial_state(wl0)
+    h0, h1 = hydro(wl0), hydro(wl1)
+    h0.upload(U0, 0); h1.upload(U0, 0)
+    h0.hydro_step(5); h1.hydro_step(5)
+    assert not np.array_equal(W.gather_valid(wl0, h0.download(0).reshape(U0.shape)),
+                              W.gather_valid(wl1, h1.download(0).reshape(U0.shape)))
+    # ... and on the shock-free config-3 recipe (p = 1 everywhere) f = 1 exactly: identical bits
+    wl0, wl1 = CASES["cfg3_periodic_small"](), flat_case("cfg3_periodic_small")
+    U0 = W.initial_state(wl0)
+    h0, h1 = hydro(wl0), hydro(wl1)
+    h0.upload(U0, 0); h1.upload(U0, 0)
+    h0.hydro_step(3); h1.hydro_step(3)
+    assert np.array_equal(W.gather_valid(wl0, h0.download(0).reshape(U0.shape)),
+                          W.gather_valid(wl1, h1.download(0).reshape(U0.shape)))
+
+
+def test_flatten_rejected_with_three_ghost_zones():
+    from paper_2007_05218_b200 import binding as B
+    wl = CASES["cfg3_ng3"]()
+    wl.params["flatten"] = 1
+    assert B.hydro_state_bytes(B.make_params(wl.params)) == 0
+
+
 def test_totals_match_oracle_on_same_state():
     wl = CASES["cfg3_periodic_small"]()
     U0 = W.initial_state(wl, ghost_value=1e30)
