@@ -72,10 +72,21 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
     # z hydro: 6 state rows with halo (ring), Lacc read, 6 components written (+ their x images),
     # F_rho written; stage 1 also reads U0 (mean over the two stages)
     out["hydro_z"] = Z * (6 * 8 * halo[2] + 5 * 8 + 6 * 8 * (1 + xend) + 8 * face[2] + 0.5 * 5 * 8)
+    if wl.params.get("flatten"):
+        # k_flatten reads (rho, m_x, m_y, m_z, rho e) with one ghost layer more than it writes; every sweep
+        # kernel reads the coefficient row of its zones (with the march halo)
+        ext = np.prod([(nb[d] + 2) / nb[d] for d in range(3)])
+        out["flatten"] = Z * (5 * 8 * np.prod([(nb[d] + 8) / nb[d] for d in range(3)]) + 8 * ext)
+        out["sweep_x"] += Z * 8 * halo[0]
+        out["hydro_y"] += Z * 8 * halo[1]
+        out["hydro_z"] += Z * 8 * halo[2]
     if ns:
         g = np.mean(ns_groups)
         out["species_y"] = Z * ((1 + g) * 8 * halo[1] + 8 * face[1] + 2 * g * 8)
         out["species_z"] = Z * ((1 + g) * 8 * halo[2] + 8 * face[2] + g * 8 + g * 8 * (1 + xend) + 0.5 * g * 8)
+        if wl.params.get("flatten"):
+            out["species_y"] += Z * 8 * halo[1]
+            out["species_z"] += Z * 8 * halo[2]
     return out
 
 
@@ -188,6 +199,8 @@ def run_ours(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=dev)
 
     wl = W.config(args.config)
+    if args.flatten:
+        wl.params["flatten"] = 1
     # ---- synthetic input, generated on the host, resident in pinned memory -------------
     t0 = time.perf_counter()
     pinned = True
@@ -299,7 +312,7 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         cfg = workload_config(wl, args.config)
         cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
-                    "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt,
+                    "flatten": bool(wl.params.get("flatten", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt,
                     "call": f"hydro_step(h, {args.steps}) -- one C-ABI call for the K timed steps",
                     "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -320,6 +333,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--flatten", action="store_true", help="switch the optional shock flattening O10 on")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -281,7 +281,9 @@ void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, in
  *   zeta = |dp| / max(small_pres, |pr[i+2] - pr[i-2]|)
  *   z    = min(1, max(0, 10*(zeta - 0.75)))                    (ramp from 0.75 to 0.85)
  *   chi  = (|dp| / min(pr[i+1], pr[i-1]) > 0.33  and  un[i-1] - un[i+1] >= 0) ? 1 : 0
- *   flat[i] = 1 - max(chi[i]*z[i], chi[i-s]*z[i-s]),  s = +1 if dp[i] > 0 else -1
+ *   flat[i] = 1 - max(chi[i]*z[i], chi[i-s]*z[i-s]),  s = +1 if dp[i] > 0, -1 if dp[i] < 0;
+ *             with dp[i] == 0 there is no high-pressure side and no neighbour is consulted (reading
+ *             F3: keeps the scheme exactly mirror-symmetric; chi[i]*z[i] is 0 there anyway)
  * z, chi are defined for i = 2 .. n-3 and flat for i = 3 .. n-4; other entries are set to 1
  * (no flattening).  flat = 1 keeps the parabola, flat = 0 replaces it by the zone average. */
 void oracle_flatten_line(const double *pr, const double *un, int n, double small_pres, double *flat)
@@ -300,8 +302,10 @@ void oracle_flatten_line(const double *pr, const double *un, int n, double small
         dpl[i] = dp;
     }
     for (int i = 3; i <= n - 4; ++i) {
-        int sft = dpl[i] > 0.0 ? 1 : -1;
-        flat[i] = 1.0 - dmax(zc[i], zc[i - sft]);
+        double nbr = 0.0;
+        if (dpl[i] > 0.0) nbr = zc[i - 1];
+        else if (dpl[i] < 0.0) nbr = zc[i + 1];
+        flat[i] = 1.0 - dmax(zc[i], nbr);
     }
     free(dpl); free(zc);
 }

@@ -44,7 +44,8 @@ __device__ __forceinline__ double flat_dir(const Geom& g, const double* __restri
     flat_zc<DIR>(g, Ub, z, st, zc0, dp0);
     flat_zc<DIR>(g, Ub, z - st, st, zcm, dpx);
     flat_zc<DIR>(g, Ub, z + st, st, zcp, dpx);
-    const double nb = dp0 > 0.0 ? zcm : zcp;          // i - s with s = +1 for dp > 0, else -1
+    // neighbour on the low-pressure side: i-1 for dp > 0, i+1 for dp < 0, none for dp == 0
+    const double nb = dp0 > 0.0 ? zcm : (dp0 < 0.0 ? zcp : 0.0);
     return 1.0 - dmax(zc0, nb);
 }
 

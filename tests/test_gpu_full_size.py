@@ -90,9 +90,11 @@ def check_windows(wl, h, dt, windows, size=40, tol=1e-11):
     return worst
 
 
-def full_run(n_cfg, threads=16):
+def full_run(n_cfg, threads=16, flatten=0):
     from paper_2007_05218_b200.binding import Hydro
     wl = W.config(n_cfg)
+    if flatten:
+        wl.params["flatten"] = 1
     U0 = W.initial_state(wl, threads=threads)
     h = Hydro(wl.params)
     h.upload(U0, 0)
@@ -155,8 +157,11 @@ def test_config3_periodic_conservation_and_windows():
     assert np.all(np.abs(t1 - t0) <= 1e-13 * scale)                 # 10 steps, BASELINE config 3
 
 
-def test_config2_sedov_windows_and_radius():
-    wl, U0, h = full_run(2)
+@pytest.mark.parametrize("flatten", [0, 1])
+def test_config2_sedov_windows_and_radius(flatten):
+    """flatten = 1: the same checks with the optional shock flattening O10 switched on (the blast is the
+    strong-shock case it exists for)."""
+    wl, U0, h = full_run(2, flatten=flatten)
     del U0
     E0 = h.hydro_conserved_totals(0)[4]
     dt = h.hydro_step(1)

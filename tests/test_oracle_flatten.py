@@ -12,11 +12,19 @@ from test_oracle_scheme import exact_riemann_sod, run_steps, run_to
 
 def test_flatten_line_strong_compressive_jump():
     # p jumps 1 -> 10 between zones 5 and 6, flow converging: |dp|/|dp2| = 1 -> z = 1, chi = 1 at zones
-    # 5 and 6; zone 4 has dp = 0 and takes its neighbour on the low-pressure side... by the sign rule
-    # s = -1 for dp <= 0 it looks at zone 5: flattened; zone 7 (dp = 0) looks at zone 8: untouched
+    # 5 and 6 (each also sees the other as its low-pressure-side neighbour); zones 4 and 7 have dp = 0:
+    # no neighbour is consulted, they keep their parabolas
     pr = np.array([1, 1, 1, 1, 1, 1, 10, 10, 10, 10, 10, 10], float)
     un = np.array([1.0] * 6 + [0.0] * 6)
-    assert np.array_equal(O.flatten_line(pr, un), [1, 1, 1, 1, 0, 0, 0, 1, 1, 1, 1, 1])
+    assert np.array_equal(O.flatten_line(pr, un), [1, 1, 1, 1, 1, 0, 0, 1, 1, 1, 1, 1])
+    # mirror image of the line (pressure and velocity reversed, velocity sign flipped): mirrored result
+    assert np.array_equal(O.flatten_line(pr[::-1].copy(), -un[::-1].copy()), [1, 1, 1, 1, 1, 0, 0, 1, 1, 1, 1, 1])
+    # a three-zone ramp 1, 4, 10: the zone below the ramp (dp > 0 towards it) is flattened through its
+    # low-pressure-side rule only if ITS neighbour on that side is a shock zone -- here zone 4 looks at 3
+    pr2 = np.array([1, 1, 1, 1, 1, 4, 10, 10, 10, 10, 10, 10], float)
+    f2 = O.flatten_line(pr2, un)
+    m2 = O.flatten_line(pr2[::-1].copy(), -un[::-1].copy())
+    assert np.array_equal(f2, m2[::-1])
     # the same jump in an expanding flow (un increasing) is not a shock
     assert np.array_equal(O.flatten_line(pr, un[::-1].copy()), np.ones(12))
 
@@ -95,3 +103,14 @@ def test_flatten_box_decomposition_invariance_bitwise():
     U = W.scatter_valid(w0, G0)
     run_steps(w0, U, 3)
     assert not np.array_equal(out[0], W.gather_valid(w0, U))
+
+
+def test_flatten_keeps_the_blast_mirror_symmetric():
+    # a point blast centred on a zone corner has mirror pairs of zones; the dp == 0 rule (reading F3) is
+    # what keeps O10 from preferring one direction
+    wl = W.config(2, ndom=(32, 32, 32), nbox=(16, 16, 32)); wl.params["flatten"] = 1
+    U = W.initial_state(wl)
+    run_steps(wl, U, 12)
+    rho = W.gather_valid(wl, U)[0]
+    assert np.allclose(rho, rho[::-1, ::-1, ::-1], rtol=1e-12, atol=0)
+    assert rho.max() > 1.5                      # the shock has formed and moved
