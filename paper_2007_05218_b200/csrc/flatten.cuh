@@ -3,9 +3,8 @@
 // written to FL (one padded array per box, laid out like a state component).  The sweeps blend the
 // monotonised parabola with the zone average:  aL <- f*aL + (1-f)*a,  aR <- f*aR + (1-f)*a.
 //
-// The coefficient contains two yes/no decisions (shock strength > 0.33, converging flow), so its
-// inputs are formed with IEEE division in BOTH builds: p = max((gamma-1)*rho_e, small_pres) and
-// u = m * (1/max(rho, small_dens)) are then bit-identical to the definition's, and so is FL.
+// The coefficient contains two yes/no decisions (shock strength > 0.33, converging flow); both are taken
+// exactly as the definition takes them (flat_zc), in both builds; the value z of the ramp is continuous.
 #pragma once
 #include "hydro_device.cuh"
 
@@ -17,50 +16,89 @@ __device__ __forceinline__ void flat_blend(double f, double omf, double a, doubl
     aR = f * aR + omf * a;
 }
 
-// chi*z and dp of padded zone index m along direction DIR of the line through (i, j, k)
+// chi*z of the zone at padded offset z along direction DIR (st = stride of DIR).
+// The two yes/no tests are filtered predicates: they are decided with the fast reciprocal when the
+// margin is far larger than its error (relative 1e-12 against <= 2 ulp), and only the rare near-ties
+// are redone with IEEE division, so the decision is always the definition's; z itself is continuous in
+// its inputs and may differ from the definition by rounding.
 template <int DIR>
-__device__ __forceinline__ void flat_zc(const Geom& g, const double* __restrict__ Ub, long long z, long long st,
-                                        double& zc, double& dp)
+__device__ __forceinline__ double flat_zc(const Geom& g, const double* __restrict__ Ub, long long z, long long st)
 {
     auto pres = [&](long long zz) { return dmax(g.gm1 * __ldg(Ub + 5 * g.cstride + zz), g.small_pres); };
-    auto vel = [&](long long zz) {
-        const double r = dmax(__ldg(Ub + zz), g.small_dens);
-        return __dmul_rn(__ldg(Ub + (1 + DIR) * g.cstride + zz), __drcp_rn(r));
-    };
     const double pm = pres(z - st), pp = pres(z + st);
-    dp = pp - pm;
+    const double adp = fabs(pp - pm);
     const double den = dmax(g.small_pres, fabs(pres(z + 2 * st) - pres(z - 2 * st)));
-    const double zeta = __ddiv_rn(fabs(dp), den);
+    const double zeta = ddiv(adp, den);
     const double zr = dmin(1.0, dmax(0.0, 10.0 * (zeta - 0.75)));
-    const bool shock = __ddiv_rn(fabs(dp), dmin(pp, pm)) > 0.33 && (vel(z - st) - vel(z + st) >= 0.0);
-    zc = shock ? zr : 0.0;
+    double zc = 0.0;
+    if (zr > 0.0) {                                    // only zones inside a steep pressure ramp go on
+        const double pmin = dmin(pp, pm);
+        const double q = adp * drcp(pmin);
+        bool strong;
+        if (fabs(q - 0.33) > 1e-12) strong = q > 0.33;
+        else strong = __ddiv_rn(adp, pmin) > 0.33;
+        if (strong) {
+            const double rm = dmax(__ldg(Ub + z - st), g.small_dens), rp = dmax(__ldg(Ub + z + st), g.small_dens);
+            const double mm = __ldg(Ub + (1 + DIR) * g.cstride + z - st), mp = __ldg(Ub + (1 + DIR) * g.cstride + z + st);
+            const double um = mm * drcp(rm), up = mp * drcp(rp);
+            const double d = um - up;
+            bool conv;
+            if (fabs(d) > 1e-12 * (fabs(um) + fabs(up))) conv = d >= 0.0;
+            else conv = __dmul_rn(mm, __drcp_rn(rm)) - __dmul_rn(mp, __drcp_rn(rp)) >= 0.0;
+            if (conv) zc = zr;
+        }
+    }
+    return zc;
 }
 
-template <int DIR>
-__device__ __forceinline__ double flat_dir(const Geom& g, const double* __restrict__ Ub, long long z)
+// Blocks of 32 x 4 x 4 zones over the cube lo .. nb+1-lo' of every box:
+// grid (ceil(n0/32), ceil(n1/4), ceil(n2/4) * boxes) with n_d the zones of the cube along d.
+constexpr int FLT_BX = 32, FLT_BY = 4, FLT_BZ = 4;
+__device__ __forceinline__ bool flat_zone(const Geom& g, int lo, int& b, long long& z)
 {
-    const long long st = DIR == 0 ? 1 : (DIR == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
-    double zc0, dp0, zcm, zcp, dpx;
-    flat_zc<DIR>(g, Ub, z, st, zc0, dp0);
-    flat_zc<DIR>(g, Ub, z - st, st, zcm, dpx);
-    flat_zc<DIR>(g, Ub, z + st, st, zcp, dpx);
-    // neighbour on the low-pressure side: i-1 for dp > 0, i+1 for dp < 0, none for dp == 0
-    const double nb = dp0 > 0.0 ? zcm : (dp0 < 0.0 ? zcp : 0.0);
-    return 1.0 - dmax(zc0, nb);
+    const int n2 = g.nb[2] - 2 * lo;
+    const int zblocks = (n2 + FLT_BZ - 1) / FLT_BZ;
+    b = blockIdx.z / zblocks;
+    const int il = blockIdx.x * FLT_BX + threadIdx.x;
+    const int jl = blockIdx.y * FLT_BY + threadIdx.y;
+    const int kl = (blockIdx.z - b * zblocks) * FLT_BZ + threadIdx.z;
+    if (il >= g.nb[0] - 2 * lo || jl >= g.nb[1] - 2 * lo || kl >= n2) return false;
+    z = ((long long)(kl + g.ng + lo) * g.nt[1] + (jl + g.ng + lo)) * g.nt[0] + (il + g.ng + lo);
+    return true;
 }
 
-// grid (ceil((nb0+2)/128) * (nb1+2), nb2+2, boxes), 128 threads: one thread per zone -1 .. nb
-__global__ void __launch_bounds__(128)
-k_flatten(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ FL)
+// pass 1: ZC[d] = chi*z along d, d = 0, 1, 2, on zones -2 .. nb+1 (three padded arrays per box)
+__global__ void __launch_bounds__(FLT_BX * FLT_BY * FLT_BZ)
+k_flatten_zc(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ ZC)
 {
-    const int xblocks = (g.nb[0] + 2 + 127) / 128;
-    const int jl = blockIdx.x / xblocks, kl = blockIdx.y;
-    const int il = (blockIdx.x - jl * xblocks) * 128 + threadIdx.x;     // 0 .. nb0+1  <->  zone -1 .. nb0
-    if (il > g.nb[0] + 1) return;
-    const int b = blockIdx.z;
-    const long long z = ((long long)(kl + g.ng - 1) * g.nt[1] + (jl + g.ng - 1)) * g.nt[0] + (il + g.ng - 1);
+    int b; long long z;
+    if (!flat_zone(g, -2, b, z)) return;
     const double* Ub = U + (long long)b * g.bstride;
-    const double f = dmin(flat_dir<0>(g, Ub, z), dmin(flat_dir<1>(g, Ub, z), flat_dir<2>(g, Ub, z)));
+    double* Zb = ZC + (long long)b * 3 * g.cstride + z;
+    Zb[0] = flat_zc<0>(g, Ub, z, 1);
+    Zb[g.cstride] = flat_zc<1>(g, Ub, z, g.nt[0]);
+    Zb[2 * g.cstride] = flat_zc<2>(g, Ub, z, (long long)g.nt[0] * g.nt[1]);
+}
+
+// pass 2: FL = min over d of 1 - max(zc_d[i], zc_d[i -+ 1]) on zones -1 .. nb; the neighbour is the one
+// on the low-pressure side (none when dp == 0, reading F3)
+__global__ void __launch_bounds__(FLT_BX * FLT_BY * FLT_BZ)
+k_flatten(const __grid_constant__ Geom g, const double* __restrict__ U, const double* __restrict__ ZC,
+          double* __restrict__ FL)
+{
+    int b; long long z;
+    if (!flat_zone(g, -1, b, z)) return;
+    const double* Pb = U + (long long)b * g.bstride + 5 * g.cstride + z;
+    const double* Zb = ZC + (long long)b * 3 * g.cstride + z;
+    double f = 1.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const long long st = d == 0 ? 1 : (d == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
+        const double dp = dmax(g.gm1 * __ldg(Pb + st), g.small_pres) - dmax(g.gm1 * __ldg(Pb - st), g.small_pres);
+        const double* Zd = Zb + d * g.cstride;
+        const double nbr = dp > 0.0 ? __ldg(Zd - st) : (dp < 0.0 ? __ldg(Zd + st) : 0.0);
+        f = dmin(f, 1.0 - dmax(__ldg(Zd), nbr));
+    }
     FL[(long long)b * g.cstride + z] = f;
 }
 

@@ -33,7 +33,7 @@ constexpr int RING_D = HYDRO_RING_D;  // depth of the TMA ring of the marching k
 thread_local std::string g_init_error = "";
 
 struct Carve {
-    size_t lacc, frho, part, totals, red, dtslot, flat, total;
+    size_t lacc, frho, part, totals, red, dtslot, flat, zc, total;
 };
 
 }  // namespace
@@ -127,6 +127,7 @@ Carve carve(const Geom &g)
     c.red = off;    off += 256;
     c.dtslot = off; off += 256;
     c.flat = off;   if (g.flatten) off += up256((size_t)g.cstride * g.nboxes * 8);   // O10 coefficients
+    c.zc = off;     if (g.flatten) off += up256((size_t)g.cstride * g.nboxes * 3 * 8); // O10 chi*z per direction
     c.total = off;
     return c;
 }
@@ -324,10 +325,17 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     a.FL = nullptr;
     if (g.flatten) {   // O10: flattening coefficients of the stage state (ghosts are filled) before any sweep
         a.FL = (const double *)(h->scratch + h->cv.flat);
-        const int xblocks = (g.nb[0] + 2 + 127) / 128;
+        auto fgrid = [&](int lo) {
+            return dim3((g.nb[0] - 2 * lo + FLT_BX - 1) / FLT_BX, (g.nb[1] - 2 * lo + FLT_BY - 1) / FLT_BY,
+                        (unsigned)(((g.nb[2] - 2 * lo + FLT_BZ - 1) / FLT_BZ) * g.nboxes));
+        };
+        double *ZC = (double *)(h->scratch + h->cv.zc);
         prof_begin(h);
-        k_flatten<<<dim3(xblocks * (g.nb[1] + 2), g.nb[2] + 2, g.nboxes), 128, 0, h->stream>>>(
-            g, a.Us, (double *)(h->scratch + h->cv.flat));
+        k_flatten_zc<<<fgrid(-2), dim3(FLT_BX, FLT_BY, FLT_BZ), 0, h->stream>>>(g, a.Us, ZC);
+        int rc0 = check_launch(h, "k_flatten_zc", K_FLATTEN);
+        if (rc0) return rc0;
+        prof_begin(h);
+        k_flatten<<<fgrid(-1), dim3(FLT_BX, FLT_BY, FLT_BZ), 0, h->stream>>>(g, a.Us, ZC, (double *)(h->scratch + h->cv.flat));
         int rc = check_launch(h, "k_flatten", K_FLATTEN);
         if (rc) return rc;
     }
