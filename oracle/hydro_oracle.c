@@ -28,7 +28,8 @@
  * P3 Sod exact solution, P4 Sedov radius, P5 PPM worked example (exact
  * rationals), P6 HLLC worked example, P7 axis permutation, P8 decomposition
  * invariance, P9 3-D = 1-D, P10 gravity closed form, P11 dt closed form, P12
- * ghost fill on index-encoded data, P13 order of accuracy.
+ * ghost fill on index-encoded data, P13 order of accuracy; optional flattening O10:
+ * tests/test_oracle_flatten.py (worked lines, exact no-op, Sod, symmetry).
  * Parity unpinned: behaviour when the small_dens / small_pres floors trigger
  * (exercised GPU-vs-oracle only).
  *
