@@ -59,7 +59,8 @@ typedef struct {
     double grav[3];
     double small_dens, small_pres;
     int32_t flatten;            /* 0: off (O1..O9 as in rounds before); 1: shock flattening O10 (needs ng >= 4) */
-    int32_t pad_;
+    int32_t evolve_eint;        /* 0: rho*e re-synchronised from rho*E after every stage (O7); 1: evolved rho*e
+                                   with a dual-energy switch, O11 */
 } oracle_params;
 
 enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2 };
@@ -84,6 +85,7 @@ static int make_geom(const oracle_params *p, geom_t *g)
     if (!p) return -1;
     if (p->ng < 3 || p->nspec < 0) return -1;
     if (p->flatten != 0 && (p->flatten != 1 || p->ng < 4)) return -1;
+    if (p->evolve_eint != 0 && p->evolve_eint != 1) return -1;
     g->nvar = 6 + p->nspec;
     g->nflux = 5 + p->nspec;
     g->nq = 5 + p->nspec;
@@ -223,8 +225,10 @@ void oracle_ppm_line(const double *a, int n, double *s, double *e, double *aL, d
 /* ---- O5 HLLC (Toro star-state form, Davis wave speeds; S6, S7, S8) ------- */
 /* dir: 0,1,2.  qL, qR: NQ primitives of the left/right face states.
  * F: NFLUX fluxes out (rho, rho*u, rho*v, rho*w, rho*E, rho*X_k). */
-void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, int nspec,
-                 const double *qL, const double *qR, double *F)
+/* O5 + the face-normal velocity of the HLLC fan (O11, reading G2): the contact speed SM between the
+ * two acoustic waves, the left / right normal velocity where the whole fan lies on one side. */
+void oracle_hllc_u(int dir, double gamma, double small_dens, double small_pres, int nspec,
+                   const double *qL, const double *qR, double *F, double *uface)
 {
     const double gm1inv = 1.0 / (gamma - 1.0);
     double rK[2], vK[2][3], pK[2], nK[2], rinvK[2], cK[2], EK[2], FK[2][5], UK[2][5];
@@ -252,8 +256,10 @@ void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, in
     double SR = dmax(nK[0] + cK[0], nK[1] + cK[1]);
     if (SL >= 0.0) {
         for (int c = 0; c < 5; ++c) F[c] = FK[0][c];
+        *uface = nK[0];
     } else if (SR <= 0.0) {
         for (int c = 0; c < 5; ++c) F[c] = FK[1][c];
+        *uface = nK[1];
     } else {
         double mL = rK[0] * (SL - nK[0]);
         double mR = rK[1] * (SR - nK[1]);
@@ -267,9 +273,17 @@ void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, in
         for (int c = 0; c < 3; ++c) Us[1 + c] = fac * (c == dir ? SM : vK[K][c]);
         Us[4] = fac * (EK[K] * rinvK[K] + (SM - nK[K]) * (SM + pK[K] / mK));
         for (int c = 0; c < 5; ++c) F[c] = FK[K][c] + S * (Us[c] - UK[K][c]);
+        *uface = SM;
     }
     for (int s = 0; s < nspec; ++s)
         F[5 + s] = F[0] * (F[0] >= 0.0 ? qL[5 + s] : qR[5 + s]);
+}
+
+void oracle_hllc(int dir, double gamma, double small_dens, double small_pres, int nspec,
+                 const double *qL, const double *qR, double *F)
+{
+    double uface;
+    oracle_hllc_u(dir, gamma, small_dens, small_pres, nspec, qL, qR, F, &uface);
 }
 
 /* ---- O2..O7 one RK stage of one box -------------------------------------- */
@@ -315,15 +329,18 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
                         const double *Us, const double *Ubase, double *Uout)
 {
     const int ng = g->ng, nq = g->nq, nflux = g->nflux, nvar = g->nvar;
+    const int evolve = p->evolve_eint;
+    const int nqx = nq + (evolve ? 1 : 0);   /* O11: e = rho*e / rho is one more reconstructed scalar (G1) */
     const size_t cs = g->comp_stride;
     /* O2: primitives on every padded zone */
-    double *q = (double *)malloc(sizeof(double) * cs * nq);
+    double *q = (double *)malloc(sizeof(double) * cs * nqx);
     double *Uc = (double *)malloc(sizeof(double) * nvar);
     double *qz = (double *)malloc(sizeof(double) * nq);
     for (size_t z = 0; z < cs; ++z) {
         for (int c = 0; c < nvar; ++c) Uc[c] = Us[c * cs + z];
         oracle_cons_to_prim(p->gamma, p->small_dens, p->small_pres, p->nspec, Uc, qz);
         for (int c = 0; c < nq; ++c) q[c * cs + z] = qz[c];
+        if (evolve) q[nq * cs + z] = Uc[5] * (1.0 / dmax(Uc[0], p->small_dens));
     }
     /* O10 (optional): multi-dimensional flattening coefficient = min over the three directions of
      * the line coefficient, on zones -1 .. nb in every direction (1 elsewhere) */
@@ -361,19 +378,21 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
     /* O3-O5: face fluxes per direction.  F[d] holds NFLUX x (faces of d),
      * face (i,j,k) of direction d = low face of valid zone (i,j,k), with the
      * index along d running 0..nb[d]. */
-    double *F[3];
+    double *F[3], *Fe[3], *Uf[3];
     size_t fdim[3][3];
     for (int d = 0; d < 3; ++d) {
         for (int e = 0; e < 3; ++e) fdim[d][e] = g->nb[e] + (e == d ? 1 : 0);
         F[d] = (double *)malloc(sizeof(double) * nflux * fdim[d][0] * fdim[d][1] * fdim[d][2]);
+        Fe[d] = (double *)malloc(sizeof(double) * fdim[d][0] * fdim[d][1] * fdim[d][2]);   /* flux of rho*e (O11) */
+        Uf[d] = (double *)malloc(sizeof(double) * fdim[d][0] * fdim[d][1] * fdim[d][2]);   /* face-normal velocity */
     }
     int nmax = 0;
     for (int d = 0; d < 3; ++d) if (g->nt[d] > nmax) nmax = g->nt[d];
-    double *line = (double *)malloc(sizeof(double) * nmax * nq);
+    double *line = (double *)malloc(sizeof(double) * nmax * nqx);
     double *sl = (double *)malloc(sizeof(double) * nmax);
     double *ed = (double *)malloc(sizeof(double) * nmax);
-    double *lL = (double *)malloc(sizeof(double) * nmax * nq);
-    double *lR = (double *)malloc(sizeof(double) * nmax * nq);
+    double *lL = (double *)malloc(sizeof(double) * nmax * nqx);
+    double *lR = (double *)malloc(sizeof(double) * nmax * nqx);
     double *fL = (double *)malloc(sizeof(double) * nq);
     double *fR = (double *)malloc(sizeof(double) * nq);
     double *Ff = (double *)malloc(sizeof(double) * nflux);
@@ -386,7 +405,7 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
             int ijk[3];
             ijk[d1] = t1 + ng;
             ijk[d2] = t2 + ng;
-            for (int c = 0; c < nq; ++c) {
+            for (int c = 0; c < nqx; ++c) {
                 for (int m = 0; m < n; ++m) {
                     ijk[d] = m - 3 + ng;
                     line[c * nmax + m] = q[c * cs + zidx(g, ijk[0], ijk[1], ijk[2])];
@@ -408,11 +427,17 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
                     fL[c] = lR[c * nmax + f + 2];
                     fR[c] = lL[c * nmax + f + 3];
                 }
-                oracle_hllc(d, p->gamma, p->small_dens, p->small_pres, p->nspec, fL, fR, Ff);
+                double uface;
+                oracle_hllc_u(d, p->gamma, p->small_dens, p->small_pres, p->nspec, fL, fR, Ff, &uface);
                 int fi[3];
                 fi[d] = f; fi[d1] = t1; fi[d2] = t2;
                 size_t fz = ((size_t)fi[2] * fdim[d][1] + fi[1]) * fdim[d][0] + fi[0];
                 for (int c = 0; c < nflux; ++c) F[d][c * fcs + fz] = Ff[c];
+                if (evolve) {   /* G1: passive upwinding of e with the mass flux, like a species (S7) */
+                    const double eL = lR[nq * nmax + f + 2], eR = lL[nq * nmax + f + 3];
+                    Fe[d][fz] = Ff[0] * (Ff[0] >= 0.0 ? eL : eR);
+                    Uf[d][fz] = uface;
+                }
             }
         }
     }
@@ -454,13 +479,31 @@ static void advance_box(const oracle_params *p, const geom_t *g, int stage, doub
                    mz = Uout[3 * cs + z], rE = Uout[4 * cs + z];
             double K = HALF * (mx * mx + my * my + mz * mz) / rho;
             double re = rE - K;
+            if (evolve) {
+                /* O11 (G3-G5): rho*e advanced by its own equation,
+                 *   d(rho e)/dt = -div(F_rho e) - p div(u_face),  p = cell pressure of the stage state,
+                 * and used instead of rho*E - K wherever the latter is a small difference of large
+                 * numbers: rho*E - K <= eta2 * rho*E, eta2 = 1e-4 (dual-energy switch) */
+                double Le = -(Fe[0][fx1] - Fe[0][fx0]) * g->dxinv[0]
+                            - (Fe[1][fy1] - Fe[1][fy0]) * g->dxinv[1]
+                            - (Fe[2][fz1] - Fe[2][fz0]) * g->dxinv[2];
+                double divu = (Uf[0][fx1] - Uf[0][fx0]) * g->dxinv[0]
+                              + (Uf[1][fy1] - Uf[1][fy0]) * g->dxinv[1]
+                              + (Uf[2][fz1] - Uf[2][fz0]) * g->dxinv[2];
+                double pc = dmax((p->gamma - 1.0) * Us[5 * cs + z], p->small_pres);
+                Le = Le - pc * divu;
+                double rev;
+                if (stage == 0) rev = Us[5 * cs + z] + dt * Le;
+                else rev = HALF * Ubase[5 * cs + z] + HALF * (Us[5 * cs + z] + dt * Le);
+                if (!(re > 1.0e-4 * rE)) re = rev;
+            }
             if (re < floor_rhoe) re = floor_rhoe;
             Uout[5 * cs + z] = re;
         }
     }
     free(L);
     free(Ff); free(fR); free(fL); free(lR); free(lL); free(ed); free(sl); free(line);
-    for (int d = 0; d < 3; ++d) free(F[d]);
+    for (int d = 0; d < 3; ++d) { free(F[d]); free(Fe[d]); free(Uf[d]); }
     free(flatn);
     free(qz); free(Uc); free(q);
 }

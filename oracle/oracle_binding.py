@@ -18,7 +18,7 @@ class OracleParams(C.Structure):
         ("prob_lo", C.c_double * 3), ("prob_hi", C.c_double * 3),
         ("gamma", C.c_double), ("cfl", C.c_double), ("grav", C.c_double * 3),
         ("small_dens", C.c_double), ("small_pres", C.c_double),
-        ("flatten", C.c_int32), ("pad_", C.c_int32),
+        ("flatten", C.c_int32), ("evolve_eint", C.c_int32),
     ]
 
 
@@ -33,6 +33,7 @@ def make_params(d: dict) -> OracleParams:
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
     p.flatten = int(d.get("flatten", 0))
+    p.evolve_eint = int(d.get("evolve_eint", 0))
     return p
 
 

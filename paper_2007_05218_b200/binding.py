@@ -40,6 +40,8 @@ def make_params(d: dict) -> HydroParams:
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
     p.flatten = int(d.get("flatten", 0))
+    if int(d.get("evolve_eint", 0)) != 0:
+        raise NotImplementedError("evolved rho*e (O11) exists in the oracle only so far")
     return p
 
 

@@ -23,7 +23,7 @@ struct Geom {
     int NB[3];       // boxes per dimension
     int ndom[3];
     int bc_lo[3], bc_hi[3];
-    int ng, nspec, nvar, nflux, nboxes, has_grav, flatten;
+    int ng, nspec, nvar, nflux, nboxes, has_grav, flatten, evolve;
     long long cstride;   // doubles per (box, component) of a state     = nt0*nt1*nt2
     long long bstride;   // doubles per box of a state                  = cstride*nvar
     long long lcstride;  // doubles per (box, component) of the accumulator = nb0*nb1*nb2
@@ -124,9 +124,10 @@ __device__ __forceinline__ double dsqrt(double x)
 
 // ---- O5: HLLC flux of (rho, rho u, rho v, rho w, rho E) at one face ------------------
 // DIR = face normal.  qL/qR = (rho, u, v, w, p) left/right states.
+// uf = face-normal velocity of the fan (O11, reading G2): SM between the acoustic waves, else the upwind n.
 template <int DIR>
 __device__ __forceinline__ void hllc(const Geom& g, const double (&qL)[5], const double (&qR)[5],
-                                     double (&F)[5])
+                                     double (&F)[5], double& uf)
 {
     const double rL = dmax(qL[0], g.small_dens), rR = dmax(qR[0], g.small_dens);
     const double pL = dmax(qL[4], g.small_pres), pR = dmax(qR[4], g.small_pres);
@@ -174,6 +175,14 @@ __device__ __forceinline__ void hllc(const Geom& g, const double (&qL)[5], const
     Us[4] = fac * (EK * rinvK + (SM - nK) * (SM + ddiv(pK, mK)));
 #pragma unroll
     for (int c = 0; c < 5; ++c) F[c] = star ? FK[c] + S * (Us[c] - UK[c]) : FK[c];
+    uf = star ? SM : nK;
+}
+
+template <int DIR>
+__device__ __forceinline__ void hllc(const Geom& g, const double (&qL)[5], const double (&qR)[5], double (&F)[5])
+{
+    double uf;
+    hllc<DIR>(g, qL, qR, F, uf);
 }
 
 // ---- O2: conserved -> primitive for the five hydro variables -------------------------
