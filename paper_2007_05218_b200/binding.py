@@ -26,7 +26,7 @@ class HydroParams(C.Structure):
         ("prob_lo", C.c_double * 3), ("prob_hi", C.c_double * 3),
         ("gamma", C.c_double), ("cfl", C.c_double), ("grav", C.c_double * 3),
         ("small_dens", C.c_double), ("small_pres", C.c_double),
-        ("flatten", C.c_int32), ("reserved_", C.c_int32),
+        ("flatten", C.c_int32), ("evolve_eint", C.c_int32),
     ]
 
 
@@ -40,8 +40,7 @@ def make_params(d: dict) -> HydroParams:
     p.gamma, p.cfl = float(d["gamma"]), float(d["cfl"])
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
     p.flatten = int(d.get("flatten", 0))
-    if int(d.get("evolve_eint", 0)) != 0:
-        raise NotImplementedError("evolved rho*e (O11) exists in the oracle only so far")
+    p.evolve_eint = int(d.get("evolve_eint", 0))
     return p
 
 

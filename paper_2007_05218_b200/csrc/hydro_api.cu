@@ -72,8 +72,10 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
     if (!(p->gamma > 1.0)) { why = "gamma must be > 1"; return false; }
     if (p->flatten != 0 && p->flatten != 1) { why = "flatten must be 0 or 1"; return false; }
     if (p->flatten == 1 && p->ng < 4) { why = "flattening needs ng >= 4"; return false; }
+    if (p->evolve_eint != 0 && p->evolve_eint != 1) { why = "evolve_eint must be 0 or 1"; return false; }
     std::memset(&g, 0, sizeof(g));
     g.flatten = p->flatten;
+    g.evolve = p->evolve_eint;
     g.ng = p->ng; g.nspec = p->nspec; g.nvar = 6 + p->nspec; g.nflux = 5 + p->nspec;
     g.nboxes = 1;
     double dx[3];
@@ -102,7 +104,9 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
     g.cstride = (long long)g.nt[0] * g.nt[1] * g.nt[2];
     g.bstride = g.cstride * g.nvar;
     g.lcstride = (long long)g.nb[0] * g.nb[1] * g.nb[2];
-    g.lbstride = g.lcstride * g.nflux;
+    // accumulator components per zone: the NFLUX flux differences; with O11 three more (flux of rho*e,
+    // div(u_face), rho*E - K of the new state)
+    g.lbstride = g.lcstride * (g.nflux + (p->evolve_eint ? 3 : 0));
     g.fbstride = (long long)(g.nb[0] + 1) * (g.nb[1] + 1) * (g.nb[2] + 1);
     g.fbstride += g.fbstride & 1;                     // keep every box's face array 16-byte aligned
     g.gamma = p->gamma; g.gm1 = p->gamma - 1.0; g.gm1inv = 1.0 / (p->gamma - 1.0);
@@ -224,6 +228,15 @@ void launch_species_ring_n(hydro_handle h, const SweepArgs &a, dim3 grid, const 
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
 
+template <int DIR, bool FINAL, int STAGE, bool FLAT>
+void launch_energy_ring(hydro_handle h, const SweepArgs &a, dim3 grid, const RingMaps &tm)
+{
+    const size_t sm = (size_t)RING_D * (2 + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
+    auto kern = k_march_species<DIR, FINAL, STAGE, 1, BS, RING_D, FLAT, FINAL>;   // ENERGY terms only in the FINAL sweep
+    static bool once = (set_smem(kern, sm), true); (void)once;
+    kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
+}
+
 template <int DIR, bool FINAL, int STAGE>
 void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, int state)
 {
@@ -243,12 +256,12 @@ void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, 
     }
 }
 
-template <int DIR, bool FINAL, int STAGE, bool FLAT>
+template <int DIR, bool FINAL, int STAGE, bool FLAT, bool EVOLVE>
 void launch_hydro_ring(hydro_handle h, const SweepArgs &a, dim3 grid, int state)
 {
     constexpr int NROW = (FINAL ? 6 : 5) + (FLAT ? 1 : 0);
     const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
-    auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D, FLAT>;
+    auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D, FLAT, EVOLVE>;
     static bool once = (set_smem(kern, sm), true); (void)once;
     RingMaps tm;
     tm.a = h->maps[state][DIR - 1][FINAL ? 6 : 4];
@@ -283,8 +296,10 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     }
     prof_begin(h);
     if (ring) {
-        if (g.flatten) launch_hydro_ring<DIR, FINAL, STAGE, true>(h, a, grid, state);
-        else launch_hydro_ring<DIR, FINAL, STAGE, false>(h, a, grid, state);
+        if (g.flatten && g.evolve) launch_hydro_ring<DIR, FINAL, STAGE, true, true>(h, a, grid, state);
+        else if (g.flatten) launch_hydro_ring<DIR, FINAL, STAGE, true, false>(h, a, grid, state);
+        else if (g.evolve) launch_hydro_ring<DIR, FINAL, STAGE, false, true>(h, a, grid, state);
+        else launch_hydro_ring<DIR, FINAL, STAGE, false, false>(h, a, grid, state);
     } else
         k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
@@ -296,12 +311,25 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
         for (int gr = 0; gr < ngroups; ++gr) {
             const int ns = base + (gr < rem ? 1 : 0);
             a.sbase = s0;
+            a.lacc_shift = 0;
             prof_begin(h);
             if (ring) launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid, state);
             else launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
             if ((rc = check_launch(h, "k_sweep_species", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
             s0 += ns;
         }
+    }
+    if (g.evolve) {   // O11: e = rho*e / rho as one more upwinded scalar (state component 5, accumulator slot nflux)
+        a.sbase = -1;
+        a.lacc_shift = g.nflux - 4;
+        prof_begin(h);
+        RingMaps tm;
+        tm.a = h->maps[state][DIR - 1][1];
+        tm.b = h->maps[state][DIR - 1][1];
+        tm.f = h->fmaps[DIR - 1];
+        if (g.flatten) launch_energy_ring<DIR, FINAL, STAGE, true>(h, a, grid, tm);
+        else launch_energy_ring<DIR, FINAL, STAGE, false>(h, a, grid, tm);
+        if ((rc = check_launch(h, "k_march_species<energy>", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
     }
     return HYDRO_OK;
 }
@@ -345,10 +373,11 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
         const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS);
         if (gx > 2147483647LL || g.nb[2] > 65535) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
         prof_begin(h);
-        if (g.flatten)
-            k_sweep_x<WARPS, true><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
-        else
-            k_sweep_x<WARPS, false><<<dim3((unsigned)gx, g.nb[2], g.nboxes), WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
+        const dim3 xg((unsigned)gx, g.nb[2], g.nboxes);
+        if (g.flatten && g.evolve) k_sweep_x<WARPS, true, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
+        else if (g.flatten) k_sweep_x<WARPS, true, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
+        else if (g.evolve) k_sweep_x<WARPS, false, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
+        else k_sweep_x<WARPS, false, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
         int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }
@@ -465,9 +494,14 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
             if (!make_ring_map(&h->fmaps[dir - 1], FL, g, dir, 1, why2, 1, g.cstride)) h->use_ring = false;
         }
     }
+    if (g.evolve && !h->use_ring) {   // O11 lives in the ring kernels only (even ng, even box width tiling the CTA)
+        delete h;
+        return fail(nullptr, HYDRO_EINVAL, "evolve_eint = 1 needs a geometry the TMA-ring kernels accept "
+                                           "(even ng, even nbox[0] that divides or is a multiple of 128)");
+    }
     {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
         const char *ed = getenv("HYDRO_FUSE_DT");
-        h->fuse_dt = h->use_ring && !(ed && atoi(ed) == 0);
+        h->fuse_dt = h->use_ring && !g.evolve && !(ed && atoi(ed) == 0);   // O11: rho*e is final only after the energy kernel
         const char *ef = getenv("HYDRO_SPLIT_GHOSTS");
         h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng &&
                           g.nb[2] >= g.ng && !(ef && atoi(ef) == 0);

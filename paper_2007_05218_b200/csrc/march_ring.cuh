@@ -185,7 +185,7 @@ __device__ __forceinline__ XEnds xends_setup(const Geom& g, bool on, int b, int 
 // ------------------------------------------------------------------------------------
 // hydro variables.  Ring rows: non-FINAL  rho, mx, my, mz (map a, 4 components) + rho*e (map b,
 // 1 component); FINAL  rho, mx, my, mz, rho*E, rho*e (map a, 6 components).
-template <int DIR, bool FINAL, int STAGE, int BS, int D, bool FLAT>
+template <int DIR, bool FINAL, int STAGE, int BS, int D, bool FLAT, bool EVOLVE>
 __global__ void __launch_bounds__(BS, RING_MINB)
 k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
@@ -241,6 +241,8 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
     const XEnds xe = xends_setup(g, FINAL && a.xends && m.active, b, m.i);
     double f1 = 1.0, f2 = 1.0;               // O10 coefficients of zones n-1, n-2 (FLAT)
+    double ufp = 0.0;                        // O11 face velocity of the previous face (EVOLVE)
+    constexpr int NOUT = EVOLVE ? 5 : 6;     // with O11 rho*e is not written here
     constexpr bool CFL = FINAL && STAGE == 1;
     const bool cfl_on = CFL && a.dt_next != nullptr;
     double tmax = 0.0;
@@ -253,10 +255,11 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         // early, independent global loads for the update of zone z
-        double lacc[5], ubase[5];
+        double lacc[5], ubase[5], ldiv = 0.0;
         if (upd) {
 #pragma unroll
             for (int c = 0; c < 5; ++c) lacc[c] = a.Lacc[lz + c * g.lcstride];
+            if (EVOLVE) ldiv = a.Lacc[lz + (long long)(g.nflux + 1) * g.lcstride];   // O11: div(u_face) so far
             if (FINAL && STAGE == 1) {
 #pragma unroll
                 for (int c = 0; c < 5; ++c) ubase[c] = a.Ubase[zo + c * g.cstride];
@@ -283,8 +286,11 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
         f2 = f1; f1 = fn;
         if (it >= 5) {
             double F[5];
-            hllc<DIR>(g, qL, qR, F);
+            double uf;
+            hllc<DIR>(g, qL, qR, F, uf);
             double out[6];
+            const double dsum = EVOLVE ? ldiv + (uf - ufp) * dinv : 0.0;
+            double eE = 0.0;
             if (upd) {
 #pragma unroll
                 for (int c = 0; c < 5; ++c) out[c] = lacc[c] - (F[c] - Fp[c]) * dinv;
@@ -303,6 +309,13 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                     for (int c = 0; c < 5; ++c) out[c] = rk_combine<STAGE>(us[c], (STAGE == 1) ? ubase[c] : 0.0, dt, out[c]);
                     const double K = ddiv(HALF * (out[1] * out[1] + out[2] * out[2] + out[3] * out[3]), out[0]);
                     double re = out[4] - K;
+                    eE = re;                    // O11: rho*E - K before the floor, for the dual-energy switch
+                    if (EVOLVE && fabs(re - 1.0e-4 * out[4]) <= 1e-12 * fabs(out[4])) {
+                        // within rounding of the switch threshold: form K exactly as the definition does, so
+                        // that the yes/no decision taken by the energy kernel is the definition's
+                        const double m2 = __dadd_rn(__dadd_rn(__dmul_rn(out[1], out[1]), __dmul_rn(out[2], out[2])), __dmul_rn(out[3], out[3]));
+                        eE = __dsub_rn(out[4], __ddiv_rn(__dmul_rn(HALF, m2), out[0]));
+                    }
                     if (re < g.floor_rhoe) re = g.floor_rhoe;
                     out[5] = re;
                     if (CFL && cfl_on && m.active) {       // O8 on the zone just formed (same code as k_estimate_dt)
@@ -321,13 +334,18 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                     if (!FINAL) {
 #pragma unroll
                         for (int c = 0; c < 5; ++c) a.Lacc[lz + c * g.lcstride] = out[c];
+                        if (EVOLVE) a.Lacc[lz + (long long)(g.nflux + 1) * g.lcstride] = dsum;
                     } else {
+                        if (EVOLVE) {   // rho*e is written by the energy kernel (k_march_species<ENERGY>)
+                            a.Lacc[lz + (long long)(g.nflux + 1) * g.lcstride] = dsum;
+                            a.Lacc[lz + (long long)(g.nflux + 2) * g.lcstride] = eE;
+                        }
 #pragma unroll
-                        for (int c = 0; c < 6; ++c) a.Uout[zo + c * g.cstride] = out[c];
+                        for (int c = 0; c < NOUT; ++c) a.Uout[zo + c * g.cstride] = out[c];
                         if (xe.single) {
                             const long long zi = zo + xe.d[0];
 #pragma unroll
-                            for (int c = 0; c < 6; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && xe.f[0]) ? -out[c] : out[c];
+                            for (int c = 0; c < NOUT; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && xe.f[0]) ? -out[c] : out[c];
                         } else if (xe.any) {
 #pragma unroll 1
                             for (int qr = 0; qr < xe.n[0] + xe.n[1]; ++qr) {
@@ -335,7 +353,7 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                                 const long long zi = zo + (qq ? xe.d[1] : xe.d[0]) + r * (qq ? xe.step[1] : xe.step[0]);
                                 const bool fq = qq ? xe.f[1] : xe.f[0];
 #pragma unroll
-                                for (int c = 0; c < 6; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && fq) ? -out[c] : out[c];
+                                for (int c = 0; c < NOUT; ++c) a.Uout[zi + c * g.cstride] = (c == 1 && fq) ? -out[c] : out[c];
                             }
                         }
                     }
@@ -343,6 +361,7 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
             }
 #pragma unroll
             for (int c = 0; c < 5; ++c) Fp[c] = F[c];
+            ufp = uf;
         }
         // release slot (it-KEEP): one CTA barrier per step, then thread 0 refills it
         __syncthreads();
@@ -355,7 +374,9 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 // ------------------------------------------------------------------------------------
 // NS passive species per thread.  Ring rows: rho (map a, 1 component) + rho*X_k, k = sbase..
 // sbase+NS-1 (map b, NS components).
-template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT>
+// ENERGY (NS = 1, FINAL, launched with sbase = -1): the one "species" is e = rho*e / rho of O11; the update adds
+// -p div(u_face) and ends with the dual-energy switch (readings G3-G5).
+template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT, bool ENERGY = false>
 __global__ void __launch_bounds__(BS, RING_MINB_S)
 k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
 {
@@ -397,7 +418,7 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
     // running offsets of zone z = m0-6+it (updated at step it) and of face n-2 = m0-5+it
-    long long lz = (long long)b * g.lbstride + (long long)(5 + sbase) * g.lcstride + flat_off<DIR>(g, m.i, m.t, m0 - 6, g.nb[DIR]);
+    long long lz = (long long)b * g.lbstride + (long long)(5 + sbase + a.lacc_shift) * g.lcstride + flat_off<DIR>(g, m.i, m.t, m0 - 6, g.nb[DIR]);
     long long fz = (long long)b * g.fbstride + flat_off<DIR>(g, m.i, m.t, m0 - 5, g.nb[DIR] + 1);
     long long zo = (long long)b * g.bstride + (long long)(6 + sbase) * g.cstride + zone_off<DIR>(g, m.i, m.t, m0 - 6);
     const double dinv = g.dxinv[DIR];
@@ -416,13 +437,18 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         const bool upd = (it >= 6);
         const double Frho = Fnext;
         if (it >= 4 && it + 1 < nsteps) Fnext = ldg(a.Frho + fz + lmstride);
-        double lacc[NS], ubase[NS];
+        double lacc[NS], ubase[NS], ldiv = 0.0, eE = 0.0, rEn = 0.0;
         if (upd) {
 #pragma unroll
             for (int v = 0; v < NS; ++v) lacc[v] = a.Lacc[lz + v * g.lcstride];
             if (FINAL && STAGE == 1) {
 #pragma unroll
                 for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo + v * g.cstride];
+            }
+            if (ENERGY) {     // div(u_face) and rho*E - K left by the z hydro kernel, and the new rho*E
+                ldiv = a.Lacc[lz + g.lcstride];
+                eE = a.Lacc[lz + 2 * g.lcstride];
+                rEn = a.Uout[zo - g.cstride];
             }
         }
         const double* slot = ring + (size_t)(it % D) * NROW * BS;
@@ -453,8 +479,16 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
             if (FINAL) {
                 const double* sz = ring + (size_t)((it + D - 3) % D) * NROW * BS;   // zone z's slot
 #pragma unroll
-                for (int v = 0; v < NS; ++v)
-                    out[v] = rk_combine<STAGE>(sz[(1 + v) * BS + tid], (STAGE == 1) ? ubase[v] : 0.0, dt, out[v]);
+                for (int v = 0; v < NS; ++v) {
+                    const double us = sz[(1 + v) * BS + tid];
+                    if (ENERGY) out[v] = out[v] - dmax(g.gm1 * us, g.small_pres) * ldiv;
+                    out[v] = rk_combine<STAGE>(us, (STAGE == 1) ? ubase[v] : 0.0, dt, out[v]);
+                    if (ENERGY) {                      // dual-energy switch, then the floor (as O7)
+                        double re = (eE > 1.0e-4 * rEn) ? eE : out[v];
+                        if (re < g.floor_rhoe) re = g.floor_rhoe;
+                        out[v] = re;
+                    }
+                }
             }
             if (m.active) {          // all stores of the step under one predicate
                 if (!FINAL) {

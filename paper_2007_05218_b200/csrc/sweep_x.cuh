@@ -43,7 +43,7 @@ __device__ __forceinline__ void ppm_lanes(double a, double f, double omf, double
     qRf = shfl_dn1(aL);                                // lanes 2..28
 }
 
-template <int WARPS, bool FLAT>
+template <int WARPS, bool FLAT, bool EVOLVE>
 __global__ void __launch_bounds__(WARPS * 32)
 k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ Lacc,
           const double* __restrict__ FL)
@@ -72,11 +72,13 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
     const double* p1 = Ub + g.cstride;
     const double* p2 = p1 + g.cstride;
     const double* p3 = p2 + g.cstride;
-    cons_to_prim(g, ldg(Ub), ldg(p1), ldg(p2), ldg(p3), ldg(p3 + 2 * g.cstride), q, rinv);
+    const double re_raw = ldg(p3 + 2 * g.cstride);
+    cons_to_prim(g, ldg(Ub), ldg(p1), ldg(p2), ldg(p3), re_raw, q, rinv);
     double qL[5], qR[5], F[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) ppm_lanes<FLAT>(q[v], fl, omf, qL[v], qR[v]);
-    hllc<0>(g, qL, qR, F);                             // face i+1/2, lanes 2..28
+    double uf;
+    hllc<0>(g, qL, qR, F, uf);                         // face i+1/2, lanes 2..28
 
     const bool store = (lane >= 3) && (lane <= 2 + XW_VALID) && (i < g.nb[0]);
     double* Lb = Lacc + (long long)b * g.lbstride + ((long long)k * g.nb[1] + j) * g.nb[0] + i;
@@ -88,6 +90,11 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
             const double acc = -(F[c] - Fm) * g.dxinv[0];
             if (store) *pa = acc;
             pa += g.lcstride;
+        }
+        if (EVOLVE) {     // O11: x part of div(u_face), accumulator slot nflux + 1
+            const double ufm = shfl_up1(uf);
+            const double D = (uf - ufm) * g.dxinv[0];
+            if (store) Lb[(long long)(g.nflux + 1) * g.lcstride] = D;
         }
     }
     // species: the loads of group n+1 are issued before group n is reconstructed, so the
@@ -133,6 +140,9 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
         load(xa);
         group(xb);
     }
+    // O11 (G1): e = rho*e / rho is reconstructed and upwinded like one more species; ps now points at
+    // accumulator slot nflux
+    if (EVOLVE) species(re_raw);
 }
 
 }  // namespace hydro

@@ -30,7 +30,7 @@ def test_header_symbols_all_exported(lib):
 
 
 def test_struct_layout_matches_header():
-    # 3+3+1+1+3+3 int32 = 56 bytes, then 3+3+1+1+3+1+1 doubles = 104 bytes, then flatten + reserved
+    # 3+3+1+1+3+3 int32 = 56 bytes, then 3+3+1+1+3+1+1 doubles = 104 bytes, then flatten + evolve_eint
     assert C.sizeof(B.HydroParams) == 56 + 104 + 8 and B.HydroParams.flatten.offset == 160
     assert B.HydroParams.prob_lo.offset == 56 and B.HydroParams.small_pres.offset == 152
 

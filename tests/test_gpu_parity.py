@@ -163,6 +163,83 @@ def test_flatten_rejected_with_three_ghost_zones():
     assert B.hydro_state_bytes(B.make_params(wl.params)) == 0
 
 
+# ---- O11 evolved rho*e with a dual-energy switch (optional, second half) ------------
+def cold_flow(nbox=(16, 16, 16), flatten=0, nspec=1):
+    """Cold supersonic flow (Mach 100-600) with density, velocity and pressure structure: rho*e / rho*E < 1e-4
+    everywhere, so the evolved branch of the switch is the one in use."""
+    wl = W.config(3, ndom=(32, 32, 32), nbox=nbox, nspec=nspec)
+    wl.params["evolve_eint"] = 1
+    wl.params["flatten"] = flatten
+    G0 = W.gather_valid(wl, W.initial_state(wl))
+    rho = G0[W.RHO]
+    vel = G0[1:4] / rho * 200.0 + np.array([300.0, -150.0, 80.0])[:, None, None, None]
+    G0[1:4] = rho * vel
+    G0[W.EINT] = 0.05 * (1.0 + 0.2 * np.sin(np.arange(32) * 2 * np.pi / 32))[None, None, :]
+    G0[W.EDEN] = G0[W.EINT] + 0.5 * rho * (vel ** 2).sum(axis=0)
+    assert (G0[W.EINT] / G0[W.EDEN]).max() < 1e-4
+    return wl, W.scatter_valid(wl, G0, ghost_value=np.nan)
+
+
+@pytest.mark.parametrize("nbox,flatten", [((16, 16, 16), 0), ((32, 16, 8), 1), ((16, 32, 32), 1)])
+def test_evolve_cold_flow_matches_oracle(nbox, flatten):
+    """Tolerances are ten times the usual ones: at Mach 100-600 the kinetic energy is 10^4-10^5 times rho*e, the
+    colliding streams shock within a step, and wherever the switch then selects rho*E - K the rounding of
+    rho*E (relative 1e-16 of 6e4) is an absolute error of ~1e-11 in a rho*e of order 1-60."""
+    wl, U0 = cold_flow(nbox, flatten)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.step_explicit()
+    assert abs(dt_g - dt_o) <= 1e-14 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-11), e
+    for s in range(2):
+        dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.hydro_step(2)
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o
+    Gg = W.gather_valid(wl, h.download(0).reshape(U0.shape))
+    Go = W.gather_valid(wl, Uo)
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-10), e
+    # both branches of the switch are in use by now (the colliding streams have shock-heated some zones), and
+    # rho*e agrees with the oracle relative to its OWN size
+    ratio = Go[W.EINT] / Go[W.EDEN]
+    assert ratio.min() < 1e-4 < ratio.max()
+    assert np.abs(Gg[W.EINT] - Go[W.EINT]).max() <= 1e-9 * np.abs(Go[W.EINT]).max()
+
+
+def test_evolve_free_stream_exact_and_switch_off_is_the_base_scheme():
+    # hypersonic uniform flow: every component, rho*e included, bitwise unchanged
+    wl = W.uniform((32, 16, 16), (16, 8, 8), 1, (1.0, 300.0, -180.0, 90.0, 0.1), bc=W.PERIODIC, X=(1.0,))
+    wl.params["evolve_eint"] = 1
+    U0 = W.initial_state(wl)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    h.hydro_step(3)
+    assert np.array_equal(W.gather_valid(wl, h.download(0).reshape(U0.shape)), W.gather_valid(wl, U0))
+    # rho*e / rho*E >> 1e-4 (config 5 recipe, Sod): the switch picks rho*E - K and the result is the base scheme's, bit for bit
+    for name in ("cfg5_scaling_small", "cfg1_sod"):
+        wl0 = CASES[name]()
+        wl1 = CASES[name](); wl1.params["evolve_eint"] = 1
+        U0 = W.initial_state(wl0)
+        h0, h1 = hydro(wl0), hydro(wl1)
+        h0.upload(U0, 0); h1.upload(U0, 0)
+        h0.hydro_step(3); h1.hydro_step(3)
+        assert np.array_equal(W.gather_valid(wl0, h0.download(0).reshape(U0.shape)),
+                              W.gather_valid(wl1, h1.download(0).reshape(U0.shape))), name
+
+
+def test_evolve_rejected_where_the_ring_kernels_cannot_run():
+    from paper_2007_05218_b200 import binding as B
+    wl = CASES["cfg3_one_species_odd_box"]()
+    wl.params["evolve_eint"] = 1
+    with pytest.raises(B.HydroError) as ei:
+        hydro(wl)
+    assert ei.value.code == B.HYDRO_EINVAL
+
+
 def test_totals_match_oracle_on_same_state():
     wl = CASES["cfg3_periodic_small"]()
     U0 = W.initial_state(wl, ghost_value=1e30)
