@@ -80,13 +80,25 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
         out["sweep_x"] += Z * 8 * halo[0]
         out["hydro_y"] += Z * 8 * halo[1]
         out["hydro_z"] += Z * 8 * halo[2]
-    if ns:
-        g = np.mean(ns_groups)
-        out["species_y"] = Z * ((1 + g) * 8 * halo[1] + 8 * face[1] + 2 * g * 8)
-        out["species_z"] = Z * ((1 + g) * 8 * halo[2] + 8 * face[2] + g * 8 + g * 8 * (1 + xend) + 0.5 * g * 8)
-        if wl.params.get("flatten"):
-            out["species_y"] += Z * 8 * halo[1]
-            out["species_z"] += Z * 8 * halo[2]
+    ev = bool(wl.params.get("evolve_eint"))
+    fl = bool(wl.params.get("flatten"))
+    if ev:
+        # O11: three more accumulator slots: flux of rho*e and div(u_face) go through x (written), y (read and
+        # written) and z (read; the z hydro kernel also writes the final div u and rho*E - K); the energy launch
+        # of each direction is a one-"species" sweep over (rho, rho*e) that is timed with the species class
+        out["sweep_x"] += Z * 2 * 8
+        out["hydro_y"] += Z * 2 * 8
+        out["hydro_z"] += Z * (8 + 2 * 8)
+    if ns or ev:
+        groups = list(ns_groups)
+        sy = [Z * ((1 + g) * 8 * halo[1] + 8 * face[1] + 2 * g * 8 + (8 * halo[1] if fl else 0)) for g in groups]
+        sz = [Z * ((1 + g) * 8 * halo[2] + 8 * face[2] + g * 8 + g * 8 * (1 + xend) + 0.5 * g * 8 + (8 * halo[2] if fl else 0))
+              for g in groups]
+        if ev:
+            sy.append(Z * (2 * 8 * halo[1] + 8 * face[1] + 2 * 8 + (8 * halo[1] if fl else 0)))
+            sz.append(Z * (2 * 8 * halo[2] + 8 * face[2] + 4 * 8 + 8 * (1 + xend) + 0.5 * 8 + (8 * halo[2] if fl else 0)))
+        out["species_y"] = float(np.mean(sy))
+        out["species_z"] = float(np.mean(sz))
     return out
 
 
@@ -201,6 +213,8 @@ def run_ours(args, rank, world, local_rank):
     wl = W.config(args.config)
     if args.flatten:
         wl.params["flatten"] = 1
+    if args.evolve:
+        wl.params["evolve_eint"] = 1
     # ---- synthetic input, generated on the host, resident in pinned memory -------------
     t0 = time.perf_counter()
     pinned = True
@@ -312,7 +326,7 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         cfg = workload_config(wl, args.config)
         cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
-                    "flatten": bool(wl.params.get("flatten", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt,
+                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt,
                     "call": f"hydro_step(h, {args.steps}) -- one C-ABI call for the K timed steps",
                     "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -334,6 +348,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--flatten", action="store_true", help="switch the optional shock flattening O10 on")
+    ap.add_argument("--evolve", action="store_true", help="switch the optional evolved rho*e O11 on")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

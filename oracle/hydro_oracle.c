@@ -30,6 +30,9 @@
  * invariance, P9 3-D = 1-D, P10 gravity closed form, P11 dt closed form, P12
  * ghost fill on index-encoded data, P13 order of accuracy; optional flattening O10:
  * tests/test_oracle_flatten.py (worked lines, exact no-op, Sod, symmetry).
+ * Optional evolved rho*e O11: tests/test_oracle_evolve.py (bitwise the base scheme where the switch is
+ * off, exact free stream where it is on, rounding of rho*E at Mach 1e6, conservation, invariance).
+ * Parity unpinned as well: the accuracy of the p div(u_face) term of O11 in the switch-on regime.
  * Parity unpinned: behaviour when the small_dens / small_pres floors trigger
  * (exercised GPU-vs-oracle only).
  *

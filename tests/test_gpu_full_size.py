@@ -181,3 +181,24 @@ def test_config2_sedov_windows_and_radius(flatten):
     assert abs(R - Rexact) <= 1.5 / 128, (R, Rexact, t)
     assert np.allclose(rho, rho[::-1, ::-1, ::-1], rtol=1e-11, atol=0)
     assert h.hydro_conserved_totals(0)[4] == pytest.approx(E0, rel=1e-12)
+
+
+def test_config3_evolve_and_flatten_are_noops_on_subsonic_smooth_flow():
+    """Config 3 at 256^3 (Mach ~0.3, p = 1): the dual-energy switch of O11 selects rho*E - K everywhere and the
+    flattening coefficient of O10 is 1 everywhere, so with both options on the whole path (three more
+    accumulator slots, energy launches, coefficient kernels, one more ring row) must reproduce the base
+    scheme bit for bit."""
+    import torch
+    from paper_2007_05218_b200.binding import Hydro
+    wl, U0, h = full_run(3)
+    w2 = W.config(3)
+    w2.params["evolve_eint"] = 1
+    w2.params["flatten"] = 1
+    h2 = Hydro(w2.params)
+    h2.U0.copy_(h.U0)
+    del U0
+    assert h.hydro_step(3) == h2.hydro_step(3)
+    ng = wl.ng
+    A, B = h.U0.view(wl.state_shape), h2.U0.view(wl.state_shape)
+    for b in range(wl.nboxes):
+        assert torch.equal(A[b, :, ng:-ng, ng:-ng, ng:-ng], B[b, :, ng:-ng, ng:-ng, ng:-ng]), b
