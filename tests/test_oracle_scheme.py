@@ -3,6 +3,7 @@ closed forms and invariants.  Nothing here comes from the CUDA path."""
 import numpy as np
 import pytest
 
+import golden_util
 from oracle import oracle_binding as O
 from paper_2007_05218_b200 import workloads as W
 
@@ -104,13 +105,14 @@ def exact_riemann_sod(gam=1.4, L=(1.0, 0.0, 1.0), R=(0.125, 0.0, 0.1)):
 def test_exact_riemann_star_values_match_paper_free_reference():
     # the textbook Sod star state (Toro table 4.2): pins the pin
     _, st = exact_riemann_sod()
-    assert st["p"] == pytest.approx(0.30313017805, rel=1e-10)
-    assert st["u"] == pytest.approx(0.92745262005, rel=1e-10)
-    assert st["rsL"] == pytest.approx(0.42631942818, rel=1e-10)
-    assert st["rsR"] == pytest.approx(0.26557371171, rel=1e-10)
-    assert st["shock"] == pytest.approx(1.75215573203, rel=1e-10)
-    assert st["head"] == pytest.approx(-1.18321595662, rel=1e-10)
-    assert st["tail"] == pytest.approx(-0.07027281256, rel=1e-9)
+    gold = golden_util.load("sod_exact.txt")
+    assert st["p"] == pytest.approx(gold["p_star"], rel=1e-10)
+    assert st["u"] == pytest.approx(gold["u_star"], rel=1e-10)
+    assert st["rsL"] == pytest.approx(gold["rho_star_L"], rel=1e-10)
+    assert st["rsR"] == pytest.approx(gold["rho_star_R"], rel=1e-10)
+    assert st["shock"] == pytest.approx(gold["shock_speed"], rel=1e-10)
+    assert st["head"] == pytest.approx(gold["rarefaction_head"], rel=1e-10)
+    assert st["tail"] == pytest.approx(gold["rarefaction_tail"], rel=1e-9)
 
 
 def sod_l1_error(N, tend=0.2):

@@ -7,6 +7,7 @@ from fractions import Fraction as Fr
 import numpy as np
 import pytest
 
+import golden_util
 from oracle import oracle_binding as O
 from paper_2007_05218_b200 import workloads as W
 
@@ -31,19 +32,21 @@ def test_ppm_worked_example_exact_rationals():
     # a[-2..3] = 0, 0, 1/10, 1, 2, 3  (line index m = zone + 2)
     a = [Fr(0), Fr(0), Fr(1, 10), Fr(1), Fr(2), Fr(3)]
     s, e, aL, aR = O.ppm_line([float(x) for x in a])
+    gold = golden_util.load("ppm_worked.txt")         # exact rationals, SURVEY 8(c) P5
     # slopes (CW 1.7-1.8): s[-1]=0, s[0]=1/5, s[1]=19/20
-    assert s[1] == 0.0
-    assert s[2] == pytest.approx(0.2, rel=2e-16)
-    assert s[3] == pytest.approx(0.95, rel=2e-16)
+    assert s[1] == float(gold["s_m1"]) == 0.0
+    assert s[2] == pytest.approx(float(gold["s_0"]), rel=2e-16)
+    assert s[3] == pytest.approx(float(gold["s_1"]), rel=2e-16)
     # edges (CW 1.6): e[-1/2]=1/60, e[1/2]=17/40, e[3/2]=179/120
-    assert e[1] == pytest.approx(float(Fr(1, 60)), rel=1e-14)
-    assert e[2] == pytest.approx(float(Fr(17, 40)), rel=1e-15)
-    assert e[3] == pytest.approx(float(Fr(179, 120)), rel=1e-15)
+    assert e[1] == pytest.approx(float(gold["e_m1half"]), rel=1e-14)
+    assert e[2] == pytest.approx(float(gold["e_1half"]), rel=1e-15)
+    assert e[3] == pytest.approx(float(gold["e_3half"]), rel=1e-15)
     # zone 0 (m=2): second CW 1.10 branch -> (1/60, 4/15); zone 1 (m=3) untouched
-    assert aL[2] == pytest.approx(float(Fr(1, 60)), rel=1e-14)
-    assert aR[2] == pytest.approx(float(Fr(4, 15)), rel=1e-14)
-    assert aL[3] == pytest.approx(float(Fr(17, 40)), rel=1e-15)
-    assert aR[3] == pytest.approx(float(Fr(179, 120)), rel=1e-15)
+    assert aL[2] == pytest.approx(float(gold["zone0_aL"]), rel=1e-14)
+    assert aR[2] == pytest.approx(float(gold["zone0_aR"]), rel=1e-14)
+    assert aL[3] == pytest.approx(float(gold["zone1_aL"]), rel=1e-15)
+    assert aR[3] == pytest.approx(float(gold["zone1_aR"]), rel=1e-15)
+    assert gold["zone0_aR"] == Fr(4, 15) and gold["e_3half"] == Fr(179, 120)
 
 
 def test_ppm_first_branch_mirror():
@@ -103,9 +106,11 @@ def test_hllc_sod_interface_worked_example():
     cL = np.sqrt(1.4)
     SM = 0.9 / (cL * 1.125)                       # (pR-pL)/(mL-mR), mL=-cL, mR=cL/8
     fac = cL / (cL + SM)                          # rho*_L
-    assert SM == pytest.approx(0.6761234037828133, rel=1e-14)
-    assert fac == pytest.approx(0.6363636363636364, rel=1e-14)
-    ref = [0.43026034786179024, 0.49090909090909085, 0.0, 0.0, 1.1617029392268339]
+    gold = golden_util.load("hllc_worked.txt")
+    assert cL == pytest.approx(gold["cL"], rel=1e-15) and np.sqrt(1.4 * 0.1 / 0.125) == pytest.approx(gold["cR"], rel=1e-15)
+    assert SM == pytest.approx(gold["SM"], rel=1e-14)
+    assert fac == pytest.approx(gold["fac"], rel=1e-14)
+    ref = [gold["F_rho"], gold["F_mx"], gold["F_my"], gold["F_mz"], gold["F_E"]]
     assert F[:5] == pytest.approx(ref, rel=1e-14, abs=0)
     assert F[5] == F[0] * 1.0                     # species upwinded from the left (F_rho > 0)
     # independent closed form: F = F_L + S_L (U*_L - U_L), F_L = (0, p, 0, 0, 0)
