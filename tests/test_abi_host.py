@@ -5,6 +5,7 @@ import ctypes as C
 import os
 import re
 
+import numpy as np
 import pytest
 
 from paper_2007_05218_b200 import binding as B
@@ -52,6 +53,20 @@ def test_size_queries_and_validation(lib):
     bad = W.config(3)
     bad.params["bc_hi"] = [1, 0, 0]
     assert B.hydro_state_bytes(B.make_params(bad.params)) == 0
+
+
+def test_option_fields_are_validated(lib):
+    ok = W.config(3)
+    for key, bad in (("flatten", 2), ("flatten", -1), ("evolve_eint", 2), ("evolve_eint", -3)):
+        w = W.config(3)
+        w.params[key] = bad
+        assert B.hydro_state_bytes(B.make_params(w.params)) == 0, (key, bad)
+    w = W.config(3); w.params["flatten"] = 1; w.params["evolve_eint"] = 1
+    p0, p1 = B.make_params(ok.params), B.make_params(w.params)
+    assert B.hydro_state_bytes(p1) == B.hydro_state_bytes(p0)
+    # flattening adds 4 padded arrays per box, the evolved energy 3 accumulator slots per zone
+    extra = B.hydro_scratch_bytes(p1) - B.hydro_scratch_bytes(p0)
+    assert extra >= 4 * ok.nboxes * int(np.prod(ok.nt)) * 8 + 3 * ok.zones * 8
 
 
 def test_null_handle_calls_fail_cleanly(lib):
