@@ -94,10 +94,13 @@ k_flatten(const __grid_constant__ Geom g, const double* __restrict__ U, const do
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const long long st = d == 0 ? 1 : (d == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
-        const double dp = dmax(g.gm1 * __ldg(Pb + st), g.small_pres) - dmax(g.gm1 * __ldg(Pb - st), g.small_pres);
         const double* Zd = Zb + d * g.cstride;
-        const double nbr = dp > 0.0 ? __ldg(Zd - st) : (dp < 0.0 ? __ldg(Zd + st) : 0.0);
-        f = dmin(f, 1.0 - dmax(__ldg(Zd), nbr));
+        // all five loads are independent (the neighbour is chosen after they return)
+        const double pp = __ldg(Pb + st), pm = __ldg(Pb - st);
+        const double zm = __ldg(Zd - st), z0 = __ldg(Zd), zp = __ldg(Zd + st);
+        const double dp = dmax(g.gm1 * pp, g.small_pres) - dmax(g.gm1 * pm, g.small_pres);
+        const double nbr = dp > 0.0 ? zm : (dp < 0.0 ? zp : 0.0);
+        f = dmin(f, 1.0 - dmax(z0, nbr));
     }
     FL[(long long)b * g.cstride + z] = f;
 }
