@@ -180,12 +180,13 @@ def cold_flow(nbox=(16, 16, 16), flatten=0, nspec=1):
     return wl, W.scatter_valid(wl, G0, ghost_value=np.nan)
 
 
-@pytest.mark.parametrize("nbox,flatten", [((16, 16, 16), 0), ((32, 16, 8), 1), ((16, 32, 32), 1)])
-def test_evolve_cold_flow_matches_oracle(nbox, flatten):
+@pytest.mark.parametrize("nbox,flatten,nspec", [((16, 16, 16), 0, 1), ((32, 16, 8), 1, 1), ((16, 32, 32), 1, 1),
+                                                ((16, 16, 32), 0, 0), ((32, 32, 16), 1, 6)])
+def test_evolve_cold_flow_matches_oracle(nbox, flatten, nspec):
     """Tolerances are ten times the usual ones: at Mach 100-600 the kinetic energy is 10^4-10^5 times rho*e, the
     colliding streams shock within a step, and wherever the switch then selects rho*E - K the rounding of
     rho*E (relative 1e-16 of 6e4) is an absolute error of ~1e-11 in a rho*e of order 1-60."""
-    wl, U0 = cold_flow(nbox, flatten)
+    wl, U0 = cold_flow(nbox, flatten, nspec)
     p = O.make_params(wl.params)
     h = hydro(wl)
     h.upload(U0, 0)
@@ -229,6 +230,24 @@ def test_evolve_free_stream_exact_and_switch_off_is_the_base_scheme():
         h0.hydro_step(3); h1.hydro_step(3)
         assert np.array_equal(W.gather_valid(wl0, h0.download(0).reshape(U0.shape)),
                               W.gather_valid(wl1, h1.download(0).reshape(U0.shape))), name
+
+
+def test_evolve_with_gravity_and_reflecting_walls_matches_oracle():
+    # config-4 recipe (subsonic: the switch stays off, but every O11 launch runs, next to gravity and reflection)
+    wl = CASES["cfg4_atmosphere_small"]()
+    wl.params["evolve_eint"] = 1
+    wl.params["flatten"] = 1
+    U0 = W.initial_state(wl, ghost_value=np.nan)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    for s in range(3):
+        dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.hydro_step(3)
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-11), e
 
 
 def test_evolve_rejected_where_the_ring_kernels_cannot_run():
