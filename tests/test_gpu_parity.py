@@ -421,6 +421,19 @@ def test_no_write_outside_the_callers_buffers(bcs):
     assert torch.equal(ref.U0, u0)
 
 
+def test_zero_steps_is_a_noop_and_negative_is_an_error():
+    from paper_2007_05218_b200 import binding as B
+    wl = CASES["cfg5_scaling_small"]()
+    U0 = W.initial_state(wl, ghost_value=3.0)
+    h = hydro(wl)
+    h.upload(U0, 0)
+    n0 = h.hydro_launch_count()
+    assert B.lib().hydro_step(h.h, 0, None) == B.HYDRO_OK
+    assert h.hydro_launch_count() == n0
+    assert np.array_equal(h.download(0).reshape(U0.shape), U0)
+    assert B.lib().hydro_step(h.h, -1, None) == B.HYDRO_EINVAL
+
+
 def test_error_codes():
     from paper_2007_05218_b200 import binding as B
     wl = W.uniform((16, 16, 16), (8, 8, 8), 0, (1, 0, 0, 0, 1))
