@@ -1,0 +1,42 @@
+"""Run by tests/test_gpu_strict.py in a subprocess with HYDRO_LIB pointing at the strict build
+(-fmad=false -DHYDRO_STRICT): three RK2 steps through the five separate C-ABI calls must reproduce the
+oracle BIT FOR BIT (every operation rounded separately, IEEE division and square root: the scheme's
+definition, DESIGN.md sec. 2 "the two builds")."""
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+import numpy as np  # noqa: E402
+
+from oracle import oracle_binding as O  # noqa: E402
+from paper_2007_05218_b200 import workloads as W  # noqa: E402
+from paper_2007_05218_b200.binding import Hydro  # noqa: E402
+
+CASES = [("cfg5_small", lambda: W.config(5, ndom=(64, 64, 64), nbox=(32, 32, 32))),
+         ("cfg1_sod", lambda: W.config(1)),
+         ("cfg4_small", lambda: W.config(4, ndom=(32, 32, 64), nbox=(16, 32, 32))),
+         ("cfg2_small", lambda: W.config(2, ndom=(48, 48, 48), nbox=(24, 24, 48))),
+         ("cfg3_odd_box", lambda: W.config(3, ndom=(54, 30, 14), nbox=(27, 15, 7), nspec=1))]
+bad = []
+for name, make in CASES:
+    for opts in ({}, {"flatten": 1}, {"flatten": 1, "evolve_eint": 1}):
+        wl = make()
+        wl.params.update(opts)
+        try:
+            h = Hydro(wl.params)
+        except Exception:
+            assert opts.get("evolve_eint"), (name, opts)       # only O11 may refuse a geometry (no ring kernels)
+            continue
+        U0 = W.initial_state(wl)
+        h.upload(U0, 0)
+        p = O.make_params(wl.params)
+        Uo, T = U0.copy(), np.zeros_like(U0)
+        dts_o = [O.step(p, Uo, T) for _ in range(3)]
+        dts_g = [h.step_explicit() for _ in range(3)]
+        G, Go = W.gather_valid(wl, h.download(0).reshape(U0.shape)), W.gather_valid(wl, Uo)
+        ok = dts_o == dts_g and np.array_equal(G, Go)
+        print(name, opts, "bitwise" if ok else "DIFFERS", flush=True)
+        if not ok:
+            bad.append((name, opts))
+sys.exit(1 if bad else 0)
