@@ -32,6 +32,9 @@
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 
+#ifndef RING_UNROLL_Z
+#define RING_UNROLL_Z 1     // unroll of the march loop of the FINAL hydro kernels (2 spills at 168 registers)
+#endif
 #ifndef RING_UNROLL_Y
 #define RING_UNROLL_Y 2     // unroll of the march loop of the non-FINAL hydro kernel
 #endif
@@ -250,7 +253,7 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 
     // two steps per trip in the y kernel: the rolling-window rotation becomes register renaming
     // (8.1 -> 7.6 ms per step at 512^3); the FINAL kernels spill when unrolled and stay at 1
-    constexpr int UNROLL = FINAL ? 1 : RING_UNROLL_Y;
+    constexpr int UNROLL = FINAL ? RING_UNROLL_Z : RING_UNROLL_Y;
 #pragma unroll UNROLL
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
