@@ -62,8 +62,8 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
     out = {}
     full = 2 * nvar * 8 * ghost_zones
     rows = 2 * nvar * 8 * row_zones
-    if split_ghosts:      # one full fill of the caller's state, then ghost-row copies
-        out["fill_ghosts"] = (full + (2 * steps - 1) * rows) / (2 * steps)
+    if split_ghosts:      # one full fill of the caller's state (two launches: x ends, ghost rows), then ghost-row copies
+        out["fill_ghosts"] = (full + (2 * steps - 1) * rows) / (2 * steps + 1)
     else:
         out["fill_ghosts"] = full
     out["estimate_dt"] = 5 * 8 * Z

@@ -114,6 +114,28 @@ __device__ __noinline__ bool dim_image(const Geom& g, int d, int bd, int l, int 
     return false;
 }
 
+// x ghost zones of the VALID rows (j, k valid): the first half of O1 in its split form when no z sweep has
+// written them (the caller's state).  One thread per ghost zone; grid (ceil(nb1 * 2ng / 256), nb2, nvar * boxes).
+__global__ void __launch_bounds__(256)
+k_fill_xends(const __grid_constant__ Geom g, double* __restrict__ U)
+{
+    const int ng2 = 2 * g.ng;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= g.nb[1] * ng2) return;
+    const int j = t / ng2, l = t - j * ng2;
+    const int k = blockIdx.y;
+    const int b = blockIdx.z / g.nvar, c = blockIdx.z - b * g.nvar;
+    const int bi = b % g.NB[0];
+    const int il = l < g.ng ? l : g.nb[0] + l;
+    bool fx;
+    const int gx = map_global(g, 0, bi * g.nb[0] + il - g.ng, fx);
+    const int sbi = gx / g.nb[0];
+    const long long row = ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0];
+    double v = U[((long long)(b + sbi - bi) * g.nvar + c) * g.cstride + row + (gx - sbi * g.nb[0] + g.ng)];
+    if (c == 1 && fx) v = -v;
+    U[((long long)b * g.nvar + c) * g.cstride + row + il] = v;
+}
+
 constexpr int GR_ROWS = 16;    // ghost rows per CTA of k_fill_ghost_rows
 
 // grid (ceil(nrows / GR_ROWS), nvar, nboxes), 256 threads.  nt[0] must be even (16-byte rows).

@@ -387,10 +387,22 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     return sweep_dir<2, true, 1>(h, a, stage);
 }
 
+int fill_ghost_rows_impl(hydro_handle h, int which);
+
 int fill_ghosts_impl(hydro_handle h, int which)
 {
     const Geom &g = h->g;
     if (g.nvar > 65535) return fail(h, HYDRO_EINVAL, "too many components for the ghost grid");
+    const char *em = getenv("HYDRO_FILL_MONOLITHIC");
+    if (h->split_ghosts && (long long)g.nvar * g.nboxes <= 65535 && g.nb[2] <= 65535 && !(em && atoi(em) != 0)) {
+        // split form (bit-identical, less index arithmetic and no 32-byte row-end gathers in the plane
+        // kernel): x ghost zones of the valid rows, then the ghost rows as whole-row copies
+        prof_begin(h);
+        k_fill_xends<<<dim3((g.nb[1] * 2 * g.ng + 255) / 256, g.nb[2], g.nvar * g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
+        int rc = check_launch(h, "k_fill_xends", K_GHOST);
+        if (rc) return rc;
+        return fill_ghost_rows_impl(h, which);
+    }
     prof_begin(h);
     k_fill_ghosts<<<dim3(g.nt[2], g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
     return check_launch(h, "k_fill_ghosts", K_GHOST);
