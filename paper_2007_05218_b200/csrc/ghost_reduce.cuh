@@ -230,24 +230,27 @@ __global__ void __launch_bounds__(256)
 k_estimate_dt(const __grid_constant__ Geom g, const double* __restrict__ U, unsigned long long* red,
               double* dtslot)
 {
-    const long long nzone = g.lcstride * g.nboxes;
+    // a warp takes whole rows (the row index is decoded once per row, not once per zone)
+    const long long nrows = (long long)g.nb[1] * g.nb[2] * g.nboxes;
+    const int wpb = blockDim.x >> 5, lane = threadIdx.x & 31;
     double tmax = 0.0;
     bool bad = false;
-    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < nzone;
-         v += (long long)gridDim.x * blockDim.x) {
-        long long r = v;
-        const int i = (int)(r % g.nb[0]); r /= g.nb[0];
+    for (long long row = (long long)blockIdx.x * wpb + (threadIdx.x >> 5); row < nrows; row += (long long)gridDim.x * wpb) {
+        long long r = row;
         const int j = (int)(r % g.nb[1]); r /= g.nb[1];
         const int k = (int)(r % g.nb[2]);
         const long long b = r / g.nb[2];
-        const double* Uz = U + b * g.bstride + ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0] + (i + g.ng);
-        double q[5], rinv;
-        cons_to_prim(g, ldg(Uz), ldg(Uz + g.cstride), ldg(Uz + 2 * g.cstride), ldg(Uz + 3 * g.cstride),
-                     ldg(Uz + 5 * g.cstride), q, rinv);
-        const double cs = sqrt(g.gamma * q[4] * rinv);
-        const double t = (fabs(q[1]) + cs) * g.dxinv[0] + (fabs(q[2]) + cs) * g.dxinv[1] + (fabs(q[3]) + cs) * g.dxinv[2];
-        if (!(t == t)) bad = true;
-        if (t > tmax) tmax = t;
+        const double* Ur = U + b * g.bstride + ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0] + g.ng;
+        for (int i = lane; i < g.nb[0]; i += 32) {
+            const double* Uz = Ur + i;
+            double q[5], rinv;
+            cons_to_prim(g, ldg(Uz), ldg(Uz + g.cstride), ldg(Uz + 2 * g.cstride), ldg(Uz + 3 * g.cstride),
+                         ldg(Uz + 5 * g.cstride), q, rinv);
+            const double cs = sqrt(g.gamma * q[4] * rinv);
+            const double t = (fabs(q[1]) + cs) * g.dxinv[0] + (fabs(q[2]) + cs) * g.dxinv[1] + (fabs(q[3]) + cs) * g.dxinv[2];
+            if (!(t == t)) bad = true;
+            if (t > tmax) tmax = t;
+        }
     }
     __shared__ unsigned long long sm[8];
     cfl_reduce_finish(g, bad, tmax, red, dtslot, sm);

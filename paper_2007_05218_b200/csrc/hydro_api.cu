@@ -424,8 +424,8 @@ double *dt_slot(hydro_handle h, int slot) { return (double *)(h->scratch + h->cv
 
 int launch_dt(hydro_handle h, int slot = 0)
 {
-    const long long nzone = h->g.lcstride * h->g.nboxes;
-    long long blocks = (nzone + 255) / 256;
+    const long long nrows = (long long)h->g.nb[1] * h->g.nb[2] * h->g.nboxes;
+    long long blocks = (nrows + 7) / 8;            // 8 warps per block, one row per warp and trip
     if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
     prof_begin(h);
     k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[0],
