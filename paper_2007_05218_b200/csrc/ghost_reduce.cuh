@@ -278,18 +278,17 @@ k_totals_partial(const __grid_constant__ Geom g, const double* __restrict__ U, d
 {
     const int c = blockIdx.y;
     const int sc = c < 5 ? c : c + 1;
-    const long long nzone = g.lcstride * g.nboxes;
+    // a warp takes whole rows (fixed assignment of rows to warps and of zones to lanes: deterministic)
+    const long long nrows = (long long)g.nb[1] * g.nb[2] * g.nboxes;
+    const int wpb = blockDim.x >> 5, lane = threadIdx.x & 31;
     double hi = 0.0, lo = 0.0;
-    for (long long v = (long long)blockIdx.x * blockDim.x + threadIdx.x; v < nzone;
-         v += (long long)gridDim.x * blockDim.x) {
-        long long r = v;
-        const int i = (int)(r % g.nb[0]); r /= g.nb[0];
+    for (long long row = (long long)blockIdx.x * wpb + (threadIdx.x >> 5); row < nrows; row += (long long)gridDim.x * wpb) {
+        long long r = row;
         const int j = (int)(r % g.nb[1]); r /= g.nb[1];
         const int k = (int)(r % g.nb[2]);
         const long long b = r / g.nb[2];
-        const double x = ldg(U + b * g.bstride + sc * g.cstride +
-                             ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0] + (i + g.ng));
-        dd_add(hi, lo, x, 0.0);
+        const double* Ur = U + b * g.bstride + sc * g.cstride + ((long long)(k + g.ng) * g.nt[1] + (j + g.ng)) * g.nt[0] + g.ng;
+        for (int i = lane; i < g.nb[0]; i += 32) dd_add(hi, lo, ldg(Ur + i), 0.0);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {

@@ -559,8 +559,8 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
     if (which != 0 && which != 1) return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
     if (!totals_host) return fail(h, HYDRO_EINVAL, "null totals_host");
     const Geom &g = h->g;
-    const long long nzone = g.lcstride * g.nboxes;
-    long long blocks = (nzone + 255) / 256;
+    const long long nrows = (long long)g.nb[1] * g.nb[2] * g.nboxes;
+    long long blocks = (nrows + 7) / 8;            // 8 warps per block, one row per warp and trip
     if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
     double *part = (double *)(h->scratch + h->cv.part);
     double *tot = (double *)(h->scratch + h->cv.totals);
