@@ -107,9 +107,13 @@ int hydro_estimate_dt(hydro_handle h, double *dt_host);
  * (fixed reduction tree, compensated).  Synchronises the stream. */
 int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
 
-/* Convenience: n whole RK2 steps = n x { estimate_dt; fill(0); stage(0); fill(1);
- * stage(1) } without host round trips (dt stays on the device).  dt_last_host (may be
- * NULL) receives the last dt; when it is non-NULL the call synchronises. */
+/* n whole RK2 steps = n x { estimate_dt; fill(0); stage(0); fill(1); stage(1) } without host round
+ * trips (dt stays on the device).  Results are bit-identical to the five separate calls; inside one
+ * call the work is arranged differently from the second step on: the z sweeps write
+ * the x ghost images of the zones they produce, so a ghost fill shrinks to whole-row copies, and the
+ * stage-1 z hydro sweep reduces the next step's dt.  Ghost zones of U0 are unspecified on return, as
+ * after the separate calls.  dt_last_host (may be NULL) receives the last dt; when it is non-NULL the
+ * call synchronises.  nsteps = 0 is a no-op; nsteps < 0 is HYDRO_EINVAL. */
 int hydro_step(hydro_handle h, int nsteps, double *dt_last_host);
 
 /* Which internal paths this handle uses (for bench accounting; they change no result):
