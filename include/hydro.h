@@ -152,6 +152,13 @@ const char *hydro_last_error(hydro_handle h);
  * measured FP64 peak. */
 int hydro_fp64_probe(double *rates_host);
 
+/* Measurement aid (no part of the path): bandwidth in GB/s of TMA tiled loads of {columns, 128 rows} boxes
+ * (columns = 2, 4 or 8 doubles) of `ncomp` (1..6) components of an FP64 array shaped like the config-5 state
+ * (1 048 576 rows, pitch 136 doubles, 128 valid columns), each thread of a 128-thread CTA owning one row --
+ * the transposing access of a thread-per-row march along the contiguous direction.  Allocates and frees its own
+ * buffers (up to 6.9 GB), default stream, synchronous. */
+int hydro_tma_probe(int columns, int ncomp, double *gbs_host);
+
 /* End-to-end entry for callers without device buffers: U_host (hydro_state_bytes, layout
  * a1, valid zones filled) is copied to the device, advanced nsteps RK2 steps, and copied
  * back in place; dt_host[0..nsteps-1] (may be NULL) receives the timesteps and

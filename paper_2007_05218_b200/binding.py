@@ -15,7 +15,7 @@ LIB_PATH = os.environ.get("HYDRO_LIB") or os.path.join(HERE, "libhydro_b200.so")
 HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
-           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host", "hydro_fp64_probe"]
+           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host", "hydro_fp64_probe", "hydro_tma_probe"]
 
 
 class HydroParams(C.Structure):
@@ -83,6 +83,7 @@ def lib():
     L.hydro_last_error.argtypes = [vp]
     L.hydro_run_host.argtypes = [pp, vp, C.c_int, dp, dp]
     L.hydro_fp64_probe.argtypes = [dp]
+    L.hydro_tma_probe.argtypes = [C.c_int, C.c_int, dp]
     _lib = L
     return L
 
@@ -102,6 +103,15 @@ def hydro_fp64_probe():
     if rc != 0:
         raise HydroError(rc, lib().hydro_last_error(None).decode())
     return {"dfma": r[0], "dadd_dmul": r[1], "dfma_with_imad": r[2]}
+
+
+def hydro_tma_probe(columns: int, ncomp: int) -> float:
+    """GB/s of TMA loads of {columns, 128 rows} boxes (include/hydro.h)."""
+    r = C.c_double(0.0)
+    rc = lib().hydro_tma_probe(columns, ncomp, C.byref(r))
+    if rc != 0:
+        raise HydroError(rc, lib().hydro_last_error(None).decode())
+    return r.value
 
 
 def hydro_run_host(p: HydroParams, U_host, nsteps: int, want_totals: bool = False):

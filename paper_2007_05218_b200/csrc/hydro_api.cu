@@ -448,6 +448,49 @@ int read_dt(hydro_handle h, double *dt_host, int slot = 0)
 
 }  // namespace
 
+namespace {
+template <int C, int D>
+int tma_probe_run(int nc, double *buf, long long rows, double *out, double *gbs)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn)
+        return fail(nullptr, HYDRO_ECUDA, "cuTensorMapEncodeTiled is not available from the driver");
+    const int pitch = 136, ncols = 128;
+    CUtensorMap tm;
+    cuuint64_t dims[3] = {(cuuint64_t)pitch, (cuuint64_t)rows, (cuuint64_t)nc};
+    cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)pitch * rows * 8};
+    cuuint32_t box[3] = {C, 128, 1}, estr[3] = {1, 1, 1};
+    if (((encode_fn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, buf, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return fail(nullptr, HYDRO_ECUDA, "hydro_tma_probe: cuTensorMapEncodeTiled failed");
+    const size_t sm = (size_t)D * nc * 128 * C * 8 + D * 8;
+    if (sm > 220 * 1024) return fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: ring does not fit in shared memory");
+    cudaFuncSetAttribute(k_tma_probe<C, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        k_tma_probe<C, D><<<(unsigned)(rows / 128), 128, sm>>>(tm, nc, ncols, out);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+            cudaEventDestroy(e0); cudaEventDestroy(e1);
+            return fail(nullptr, HYDRO_ECUDA, "hydro_tma_probe: kernel failed");
+        }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *gbs = (double)rows * ncols * 8 * nc / (best * 1e-3) / 1e9;
+    return HYDRO_OK;
+}
+}  // namespace
+
 extern "C" {
 
 size_t hydro_state_bytes(const hydro_params *p)
@@ -679,6 +722,27 @@ int hydro_fp64_probe(double *rates_host)
     }
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(out);
+    return rc;
+}
+
+int hydro_tma_probe(int columns, int ncomp, double *gbs_host)
+{
+    if (!gbs_host || ncomp < 1 || ncomp > 6) return fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: ncomp must be 1..6");
+    const long long rows = 128LL * 128 * 64;                       // valid rows of one component of config 5
+    double *buf = nullptr, *out = nullptr;
+    if (cudaMalloc(&buf, (size_t)136 * rows * ncomp * 8) != cudaSuccess || cudaMalloc(&out, (size_t)rows * 8) != cudaSuccess) {
+        if (buf) cudaFree(buf);
+        return fail(nullptr, HYDRO_ENOMEM, "hydro_tma_probe: device allocation failed");
+    }
+    cudaMemset(buf, 0, (size_t)136 * rows * ncomp * 8);
+    int rc;
+    switch (columns) {
+        case 2: rc = tma_probe_run<2, 8>(ncomp, buf, rows, out, gbs_host); break;
+        case 4: rc = tma_probe_run<4, 6>(ncomp, buf, rows, out, gbs_host); break;
+        case 8: rc = tma_probe_run<8, 4>(ncomp, buf, rows, out, gbs_host); break;
+        default: rc = fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: columns must be 2, 4 or 8");
+    }
+    cudaFree(out); cudaFree(buf);
     return rc;
 }
 

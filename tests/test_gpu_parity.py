@@ -434,6 +434,15 @@ def test_zero_steps_is_a_noop_and_negative_is_an_error():
     assert B.lib().hydro_step(h.h, -1, None) == B.HYDRO_EINVAL
 
 
+def test_tma_probe_runs_and_rejects_bad_arguments():
+    from paper_2007_05218_b200 import binding as B
+    assert B.hydro_tma_probe(4, 2) > 1000.0                       # GB/s; 5-6 TB/s on a healthy B200
+    with pytest.raises(B.HydroError):
+        B.hydro_tma_probe(3, 2)
+    with pytest.raises(B.HydroError):
+        B.hydro_tma_probe(4, 7)
+
+
 def test_error_codes():
     from paper_2007_05218_b200 import binding as B
     wl = W.uniform((16, 16, 16), (8, 8, 8), 0, (1, 0, 0, 0, 1))
