@@ -31,8 +31,11 @@
  * ghost fill on index-encoded data, P13 order of accuracy; optional flattening O10:
  * tests/test_oracle_flatten.py (worked lines, exact no-op, Sod, symmetry).
  * Optional evolved rho*e O11: tests/test_oracle_evolve.py (bitwise the base scheme where the switch is
- * off, exact free stream where it is on, rounding of rho*E at Mach 1e6, conservation, invariance).
- * Parity unpinned as well: the accuracy of the p div(u_face) term of O11 in the switch-on regime.
+ * off, exact free stream where it is on, rounding of rho*E at Mach 1e6, conservation, invariance) and
+ * tests/test_oracle_evolve_pins.py (P14: adiabatic compression of a hypersonic linear velocity field,
+ * rho*e_1 = rho*e_0 (1 + gamma A dt) after one stage and the Heun closed form after two -- fixes the sign
+ * of p_c div(u_face), the state p_c is taken from and every direction's dxinv; P15: a step in e moved by
+ * the upwinded mass flux only -- fixes the side F_e takes e from).
  * Parity unpinned: behaviour when the small_dens / small_pres floors trigger
  * (exercised GPU-vs-oracle only).
  *
