@@ -46,7 +46,7 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
+def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt, xmarch=False):
     """Algorithmic HBM bytes per launch of each kernel class: what the kernel
     split must move -- every input once with the 3-zone PPM halo along the sweep direction, every
     output once.  Returns {class: mean bytes per launch over the launches of `steps` steps issued
@@ -68,6 +68,12 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt):
         out["fill_ghosts"] = full
     out["estimate_dt"] = 5 * 8 * Z
     out["sweep_x"] = Z * ((nvar - 1) * 8 * halo[0] + nflux * 8)
+    if xmarch:
+        # marching x kernels (march_x.cuh): rows are read in 4-zone steps -4 .. nb0+3; the hydro launch writes
+        # F_rho,x (rows of nb0+4), every species launch reads it and rho again.  Mean over the 1 + groups launches.
+        hx, fx = (nb[0] + 8) / nb[0], (nb[0] + 4) / nb[0]
+        per = [5 * 8 * hx + 5 * 8 + 8 * fx] + [(1 + g) * 8 * hx + 8 * fx + g * 8 for g in ns_groups]
+        out["sweep_x"] = Z * float(np.mean(per))
     out["hydro_y"] = Z * (5 * 8 * halo[1] + 2 * 5 * 8 + 8 * face[1])
     # z hydro: 6 state rows with halo (ring), Lacc read, 6 components written (+ their x images),
     # F_rho written; stage 1 also reads U0 (mean over the two stages)
@@ -240,19 +246,22 @@ def run_ours(args, rank, world, local_rank):
     sampler.start()
     launches0 = h.hydro_launch_count()
     ns_max, split_ghosts, fuse_dt = h.hydro_query(3), bool(h.hydro_query(1)), bool(h.hydro_query(2))
-    h.hydro_profile(1)
+    xmarch = bool(h.hydro_query(4))
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(h.stream)
-    h.hydro_step(args.steps, want_dt=False)          # K whole RK2 steps, one C-ABI call
+    h.hydro_step(args.steps, want_dt=False)          # K whole RK2 steps, one C-ABI call; no per-launch events here
     e1.record(h.stream)
     barrier()
     ms_total = e0.elapsed_time(e1)
-    sampler.stop_flag = True
-    sampler.join(timeout=10)
+    launches = h.hydro_launch_count() - launches0
+    # per-class launch durations: the same call once more, with the library's event pairs around every launch
+    h.hydro_profile(1)
+    h.hydro_step(args.steps, want_dt=False)
     prof = h.hydro_profile_read()
     h.hydro_profile(0)
-    launches = h.hydro_launch_count() - launches0
+    sampler.stop_flag = True
+    sampler.join(timeout=10)
     dt_last = h.hydro_estimate_dt()
     totals = h.hydro_conserved_totals(0)
     ms_total = reduce_max(ms_total, world, dev)
@@ -263,7 +272,7 @@ def run_ours(args, rank, world, local_rank):
     peak, peak_src = measured_peaks()
     ngroups = max(1, -(-wl.nspec // ns_max)) if wl.nspec else 0
     groups = [wl.nspec // ngroups + (1 if i < wl.nspec % ngroups else 0) for i in range(ngroups)] if ngroups else []
-    alg = algorithmic_bytes(wl, groups, args.steps, split_ghosts, fuse_dt)
+    alg = algorithmic_bytes(wl, groups, args.steps, split_ghosts, fuse_dt, xmarch)
     kernels = {}
     tot_ms = sum(v[0] for v in prof.values())
     for k, (ms, cnt) in prof.items():
@@ -282,7 +291,7 @@ def run_ours(args, rank, world, local_rank):
     # ncu figures of the committed capture (profiles/traffic.json): DRAM bytes and instruction counts per
     # launch.  With the live launch durations they give the second roofline: FP64 pipe and issue slots.
     tr = os.path.join(ROOT, "profiles", "traffic.json")
-    fp64 = B.hydro_fp64_probe()                               # measured FP64 instr/s of this GPU, now
+    fp64 = B.hydro_probe_fp64()                               # measured FP64 instr/s of this GPU, now
     sm_max_hz = (sampler.summary().get("sm_max_mhz") or 1965.0) * 1e6
     if os.path.exists(tr):
         try:
@@ -296,7 +305,7 @@ def run_ours(args, rank, world, local_rank):
                     v["issue_slot_frac"] = wi / sec / (148 * 4 * sm_max_hz)
         except Exception:
             pass
-    roofline["alu"] = {"fp64_peak_instr_per_s": fp64["dfma"], "fp64_peak_source": "hydro_fp64_probe (independent DFMA chains), this run",
+    roofline["alu"] = {"fp64_peak_instr_per_s": fp64["dfma"], "fp64_peak_source": "hydro_probe_fp64 (libhydro_probe_b200: independent DFMA chains), this run",
                        "fp64_pipe_frac": kernels[dom].get("fp64_pipe_frac"), "issue_slot_frac": kernels[dom].get("issue_slot_frac"),
                        "note": "instruction counts from the committed ncu capture (profiles/traffic.json), durations live"}
 
@@ -326,7 +335,7 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         cfg = workload_config(wl, args.config)
         cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
-                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt,
+                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt, "x_sweep": "marching (march_x.cuh)" if xmarch else "lane-parallel (sweep_x.cuh)",
                     "call": f"hydro_step(h, {args.steps}) -- one C-ABI call for the K timed steps",
                     "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -44,7 +44,8 @@ extern "C" {
 #define HYDRO_ENOMEM  -2  /* scratch_bytes too small (or device allocation failed in
                              hydro_run_host)                                                 */
 #define HYDRO_ECUDA   -3  /* CUDA launch/runtime error; text via hydro_last_error            */
-#define HYDRO_ESTATE  -4  /* estimate_dt met a non-finite or non-positive max signal speed   */
+#define HYDRO_ESTATE  -4  /* a CFL reduction (hydro_estimate_dt, or any step of hydro_step) met a
+                             non-finite or non-positive max signal speed                     */
 
 #define HYDRO_BC_PERIODIC 0
 #define HYDRO_BC_OUTFLOW  1
@@ -76,12 +77,26 @@ size_t hydro_state_bytes(const hydro_params *p);
 size_t hydro_scratch_bytes(const hydro_params *p);
 
 /* Create a handle.  U0_dev, U1_dev: two states of hydro_state_bytes each; scratch_dev:
- * at least hydro_scratch_bytes; all 16-byte aligned, all caller-owned device memory that
- * must outlive the handle.  cuda_stream: a cudaStream_t (NULL = legacy default stream);
- * every kernel of this handle is enqueued on it.  The library allocates a few bytes of
- * pinned host memory for scalar read-back here and nothing afterwards.
+ * at least hydro_scratch_bytes; all 16-byte aligned, all caller-owned DEVICE memory on ONE
+ * device that must outlive the handle (HYDRO_EINVAL otherwise).  That device is the handle's:
+ * every later call on the handle makes it current for its own duration and restores the
+ * caller's device before it returns, so handles on several devices can live in one process.
+ * cuda_stream: a cudaStream_t of that device (NULL = legacy default stream); every kernel of
+ * this handle is enqueued on it.  The library allocates 16 KB of pinned host memory for scalar
+ * read-back here and nothing afterwards, hydro_profile(h, 1) excepted.
  * The caller writes the initial state (all NVAR components of the valid zones; ghosts
- * may hold anything) into U0 before the first step, with rho*e consistent with rho*E. */
+ * may hold anything) into U0 before the first step, with rho*e consistent with rho*E.
+ *
+ * Tuning switches, read from the environment ONCE, here (they select among internal code paths
+ * that give bit-identical results; defaults in brackets; hydro_query reports what a handle uses):
+ *   HYDRO_RING=0            plain-load y/z sweeps instead of the TMA-ring marching kernels   [1]
+ *   HYDRO_XMARCH=1          x sweep by the thread-per-row marching kernels of march_x.cuh instead of the
+ *                           lane-parallel k_sweep_x (measured equal in time, profiles/r02_xmarch.md)  [0]
+ *   HYDRO_SEGLEN=n          zones per pencil segment of the y/z sweeps                       [auto]
+ *   HYDRO_NSMAX=n           passive species per thread and launch, 1..5                      [5]
+ *   HYDRO_FUSE_DT=0         hydro_step runs k_estimate_dt every step                         [1]
+ *   HYDRO_SPLIT_GHOSTS=0    hydro_step / hydro_fill_ghosts use the one-launch ghost fill     [1]
+ *   HYDRO_FILL_MONOLITHIC=1 hydro_fill_ghosts alone uses the one-launch ghost fill           [0] */
 int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_dev,
                size_t scratch_bytes, void *cuda_stream, hydro_handle *out);
 
@@ -112,16 +127,22 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
  * call the work is arranged differently from the second step on: the z sweeps write
  * the x ghost images of the zones they produce, so a ghost fill shrinks to whole-row copies, and the
  * stage-1 z hydro sweep reduces the next step's dt.  Ghost zones of U0 are unspecified on return, as
- * after the separate calls.  dt_last_host (may be NULL) receives the last dt; when it is non-NULL the
- * call synchronises.  nsteps = 0 is a no-op; nsteps < 0 is HYDRO_EINVAL. */
-int hydro_step(hydro_handle h, int nsteps, double *dt_last_host);
+ * after the separate calls.
+ * dt_host: NULL, or HOST memory for nsteps doubles that receive the dt of every step (a driver that
+ * tracks simulation time needs them all).  Every step leaves its (dt, max signal speed) pair on the
+ * device; after the last launch the call synchronises the stream, reads the pairs back in one copy and
+ * returns HYDRO_ESTATE if ANY step's maximum was not a positive finite number (the state is then
+ * unusable), with or without dt_host.  nsteps = 0 is a no-op; nsteps < 0 is HYDRO_EINVAL. */
+int hydro_step(hydro_handle h, int nsteps, double *dt_host);
 
 /* Which internal paths this handle uses (for bench accounting; they change no result):
  * what = 0: TMA-ring marching kernels (1) or the plain-load fallback (0);
  *        1: hydro_step fills ghosts in two parts (x images written by the z sweeps + ghost-row
  *           copies) instead of one k_fill_ghosts launch per stage;
  *        2: hydro_step reduces the next step's dt inside the stage-1 z hydro sweep;
- *        3: passive species per thread and launch in the y/z species sweeps.
+ *        3: passive species per thread and launch in the species sweeps;
+ *        4: the x sweep runs as marching kernels (a thread per row, march_x.cuh; 1) or as the
+ *           lane-parallel k_sweep_x (0).
  * Returns -1 for a NULL handle or an unknown `what`. */
 int hydro_query(hydro_handle h, int what);
 
@@ -130,6 +151,8 @@ long long hydro_launch_count(hydro_handle h);
 
 /* Optional per-launch timing for measurement (bench.py's roofline object).  While enabled,
  * every kernel launch of this handle is bracketed by a CUDA event pair on the handle's stream.
+ * hydro_profile(h, 1) creates a pool of 8192 events on first use (the only allocation outside
+ * hydro_init); recording stops silently when the pool is used up and resumes after the next read.
  * hydro_profile_read synchronises, then writes the summed device time in ms and the launch
  * count of each kernel class into ms_host[HYDRO_NCLASS] / count_host[HYDRO_NCLASS] and clears the record.
  * Classes: 0 ghost fill, 1 dt reduction, 2 x sweep, 3 y hydro sweep, 4 y species sweep,
@@ -143,21 +166,6 @@ int hydro_destroy(hydro_handle h);
 /* Message of the last error on this handle; with h == NULL, of the last failed
  * hydro_init / hydro_run_host on this thread.  Never NULL. */
 const char *hydro_last_error(hydro_handle h);
-
-/* Measurement aid (no part of the path): times three small kernels on the current device and
- * writes FP64 instructions per second (thread instructions; x2 = FLOP/s for an FMA) into
- * rates_host[3]: [0] independent DFMA chains, [1] DADD/DMUL chains (no FMA), [2] DFMA chains with
- * one independent integer multiply-add between consecutive DFMAs (counts the DFMAs only).
- * Synchronous, default stream, allocates and frees 2.4 MB.  DESIGN.md sec. 5 uses [0] as the
- * measured FP64 peak. */
-int hydro_fp64_probe(double *rates_host);
-
-/* Measurement aid (no part of the path): bandwidth in GB/s of TMA tiled loads of {columns, 128 rows} boxes
- * (columns = 2, 4 or 8 doubles) of `ncomp` (1..6) components of an FP64 array shaped like the config-5 state
- * (1 048 576 rows, pitch 136 doubles, 128 valid columns), each thread of a 128-thread CTA owning one row --
- * the transposing access of a thread-per-row march along the contiguous direction.  Allocates and frees its own
- * buffers (up to 6.9 GB), default stream, synchronous. */
-int hydro_tma_probe(int columns, int ncomp, double *gbs_host);
 
 /* End-to-end entry for callers without device buffers: U_host (hydro_state_bytes, layout
  * a1, valid zones filled) is copied to the device, advanced nsteps RK2 steps, and copied

@@ -15,7 +15,9 @@ LIB_PATH = os.environ.get("HYDRO_LIB") or os.path.join(HERE, "libhydro_b200.so")
 HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
-           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host", "hydro_fp64_probe", "hydro_tma_probe"]
+           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
+PROBE_LIB_PATH = os.path.join(HERE, "libhydro_probe_b200.so")
+PROBE_EXPORTS = ["hydro_probe_fp64"]
 
 
 class HydroParams(C.Structure):
@@ -82,8 +84,6 @@ def lib():
     L.hydro_last_error.restype = C.c_char_p
     L.hydro_last_error.argtypes = [vp]
     L.hydro_run_host.argtypes = [pp, vp, C.c_int, dp, dp]
-    L.hydro_fp64_probe.argtypes = [dp]
-    L.hydro_tma_probe.argtypes = [C.c_int, C.c_int, dp]
     _lib = L
     return L
 
@@ -96,22 +96,27 @@ def hydro_scratch_bytes(p: HydroParams) -> int:
     return lib().hydro_scratch_bytes(C.byref(p))
 
 
-def hydro_fp64_probe():
-    """FP64 thread-instructions per second of the three probe kernels (include/hydro.h)."""
+_probe = None
+
+
+def probe_lib():
+    """Load libhydro_probe_b200.so (include/hydro_probe.h): bench.py's measurement aid, not the product."""
+    global _probe
+    if _probe is None:
+        if not os.path.exists(PROBE_LIB_PATH):
+            raise ImportError(f"{PROBE_LIB_PATH} is missing: run `python -m paper_2007_05218_b200.build`")
+        _probe = C.CDLL(PROBE_LIB_PATH)
+        _probe.hydro_probe_fp64.argtypes = [C.POINTER(C.c_double)]
+    return _probe
+
+
+def hydro_probe_fp64():
+    """FP64 thread-instructions per second of the three probe kernels (include/hydro_probe.h)."""
     r = (C.c_double * 3)()
-    rc = lib().hydro_fp64_probe(r)
+    rc = probe_lib().hydro_probe_fp64(r)
     if rc != 0:
-        raise HydroError(rc, lib().hydro_last_error(None).decode())
+        raise HydroError(rc, "hydro_probe_fp64 failed")
     return {"dfma": r[0], "dadd_dmul": r[1], "dfma_with_imad": r[2]}
-
-
-def hydro_tma_probe(columns: int, ncomp: int) -> float:
-    """GB/s of TMA loads of {columns, 128 rows} boxes (include/hydro.h)."""
-    r = C.c_double(0.0)
-    rc = lib().hydro_tma_probe(columns, ncomp, C.byref(r))
-    if rc != 0:
-        raise HydroError(rc, lib().hydro_last_error(None).decode())
-    return r.value
 
 
 def hydro_run_host(p: HydroParams, U_host, nsteps: int, want_totals: bool = False):
@@ -139,13 +144,14 @@ class Hydro:
             raise HydroError(HYDRO_EINVAL, "invalid hydro_params")
         self.device = torch.device(device)
         self.nflux = 5 + self.p.nspec
-        self.U0 = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
-        self.U1 = torch.zeros(sb // 8, dtype=torch.float64, device=self.device)
-        self.scratch = torch.empty(scb, dtype=torch.uint8, device=self.device)
-        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.h = C.c_void_p()
-        rc = L.hydro_init(C.byref(self.p), self.U0.data_ptr(), self.U1.data_ptr(), self.scratch.data_ptr(),
-                          scb, self.stream.cuda_stream, C.byref(self.h))
+        with torch.cuda.device(self.device):
+            self.U0 = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
+            self.U1 = torch.zeros(sb // 8, dtype=torch.float64, device=self.device)
+            self.scratch = torch.empty(scb, dtype=torch.uint8, device=self.device)
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            rc = L.hydro_init(C.byref(self.p), self.U0.data_ptr(), self.U1.data_ptr(), self.scratch.data_ptr(),
+                              scb, self.stream.cuda_stream, C.byref(self.h))
         if rc != 0:
             raise HydroError(rc, L.hydro_last_error(None).decode())
 
@@ -178,10 +184,13 @@ class Hydro:
         self._check(lib().hydro_conserved_totals(self.h, which, out))
         return list(out)
 
-    def hydro_step(self, nsteps=1, want_dt=True):
-        out = C.c_double(0.0)
-        self._check(lib().hydro_step(self.h, nsteps, C.byref(out) if want_dt else None))
-        return out.value if want_dt else None
+    def hydro_step(self, nsteps=1, want_dt=True, all_dts=False):
+        """nsteps RK2 steps in one call.  Returns the last dt (want_dt), every dt (all_dts) or None."""
+        out = (C.c_double * max(nsteps, 1))()
+        self._check(lib().hydro_step(self.h, nsteps, out if (want_dt or all_dts) else None))
+        if all_dts:
+            return list(out)[:nsteps]
+        return out[nsteps - 1] if (want_dt and nsteps > 0) else (0.0 if want_dt else None)
 
     def hydro_launch_count(self):
         return lib().hydro_launch_count(self.h)

@@ -52,16 +52,16 @@ __device__ __forceinline__ double flat_zc(const Geom& g, const double* __restric
 }
 
 // Blocks of 32 x 4 x 4 zones over the cube lo .. nb+1-lo' of every box:
-// grid (ceil(n0/32), ceil(n1/4), ceil(n2/4) * boxes) with n_d the zones of the cube along d.
+// grid (ceil(n0/32) * boxes, ceil(n1/4), ceil(n2/4)) with n_d the zones of the cube along d.
 constexpr int FLT_BX = 32, FLT_BY = 4, FLT_BZ = 4;
 __device__ __forceinline__ bool flat_zone(const Geom& g, int lo, int& b, long long& z)
 {
     const int n2 = g.nb[2] - 2 * lo;
-    const int zblocks = (n2 + FLT_BZ - 1) / FLT_BZ;
-    b = blockIdx.z / zblocks;
-    const int il = blockIdx.x * FLT_BX + threadIdx.x;
+    const int xblocks = gridDim.x / g.nboxes;
+    b = blockIdx.x / xblocks;
+    const int il = (blockIdx.x - b * xblocks) * FLT_BX + threadIdx.x;
     const int jl = blockIdx.y * FLT_BY + threadIdx.y;
-    const int kl = (blockIdx.z - b * zblocks) * FLT_BZ + threadIdx.z;
+    const int kl = blockIdx.z * FLT_BZ + threadIdx.z;
     if (il >= g.nb[0] - 2 * lo || jl >= g.nb[1] - 2 * lo || kl >= n2) return false;
     z = ((long long)(kl + g.ng + lo) * g.nt[1] + (jl + g.ng + lo)) * g.nt[0] + (il + g.ng + lo);
     return true;

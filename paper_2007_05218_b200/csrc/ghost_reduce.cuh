@@ -19,7 +19,7 @@ __device__ __forceinline__ int map_global(const Geom& g, int d, int gi, bool& fl
     return gi < 0 ? -1 - gi : 2 * n - 1 - gi;
 }
 
-// One CTA per (padded k-plane, component, box); the plane's ghost zones are enumerated as a
+// One CTA per (padded k-plane, box, component): grid (nt2 * boxes, nvar); the plane's ghost zones are enumerated as a
 // flat task list so that consecutive threads touch consecutive zones.  A plane in the ghost
 // k-range is filled whole; a plane in the valid k-range has 2*ng whole ghost rows plus the
 // 2*ng end zones of each valid row.  The k mapping is done once per CTA.  Reads valid zones,
@@ -27,7 +27,7 @@ __device__ __forceinline__ int map_global(const Geom& g, int d, int gi, bool& fl
 __global__ void __launch_bounds__(256)
 k_fill_ghosts(const __grid_constant__ Geom g, double* __restrict__ U)
 {
-    const int kl = blockIdx.x, c = blockIdx.y, b = blockIdx.z;
+    const int b = blockIdx.x / g.nt[2], kl = blockIdx.x - b * g.nt[2], c = blockIdx.y;
     const int bi = b % g.NB[0], bj = (b / g.NB[0]) % g.NB[1], bk = b / (g.NB[0] * g.NB[1]);
     bool fz;
     const int gz = map_global(g, 2, bk * g.nb[2] + kl - g.ng, fz);
@@ -115,16 +115,17 @@ __device__ __noinline__ bool dim_image(const Geom& g, int d, int bd, int l, int 
 }
 
 // x ghost zones of the VALID rows (j, k valid): the first half of O1 in its split form when no z sweep has
-// written them (the caller's state).  One thread per ghost zone; grid (ceil(nb1 * 2ng / 256), nb2, nvar * boxes).
+// written them (the caller's state).  One thread per ghost zone; grid (ceil(nb1 * 2ng / 256) * boxes, nb2, nvar).
 __global__ void __launch_bounds__(256)
 k_fill_xends(const __grid_constant__ Geom g, double* __restrict__ U)
 {
     const int ng2 = 2 * g.ng;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int xblocks = gridDim.x / g.nboxes;
+    const int b = blockIdx.x / xblocks, c = blockIdx.z;
+    const int t = (blockIdx.x - b * xblocks) * blockDim.x + threadIdx.x;
     if (t >= g.nb[1] * ng2) return;
     const int j = t / ng2, l = t - j * ng2;
     const int k = blockIdx.y;
-    const int b = blockIdx.z / g.nvar, c = blockIdx.z - b * g.nvar;
     const int bi = b % g.NB[0];
     const int il = l < g.ng ? l : g.nb[0] + l;
     bool fx;
@@ -138,16 +139,17 @@ k_fill_xends(const __grid_constant__ Geom g, double* __restrict__ U)
 
 constexpr int GR_ROWS = 16;    // ghost rows per CTA of k_fill_ghost_rows
 
-// grid (ceil(nrows / GR_ROWS), nvar, nboxes), 256 threads.  nt[0] must be even (16-byte rows).
+// grid (ceil(nrows / GR_ROWS) * boxes, nvar), 256 threads.  nt[0] must be even (16-byte rows).
 __global__ void __launch_bounds__(256)
 k_fill_ghost_rows(const __grid_constant__ Geom g, double* __restrict__ U)
 {
     __shared__ long long s_src[GR_ROWS], s_dst[GR_ROWS];
     __shared__ double s_sgn[GR_ROWS];
-    const int c = blockIdx.y, b = blockIdx.z;
+    const int rblocks = gridDim.x / g.nboxes;
+    const int b = blockIdx.x / rblocks, c = blockIdx.y;
     const int ng2 = 2 * g.ng;
     const int nrows = g.nt[2] * g.nt[1] - g.nb[2] * g.nb[1];
-    const int r0 = blockIdx.x * GR_ROWS;
+    const int r0 = (blockIdx.x - b * rblocks) * GR_ROWS;
     if (threadIdx.x < GR_ROWS) {
         const int r = r0 + threadIdx.x;
         long long src = -1, dst = 0;
@@ -319,33 +321,6 @@ k_totals_final(const __grid_constant__ Geom g, const double* __restrict__ part, 
         dd_add(hi, lo, oh, ol);
     }
     if (threadIdx.x == 0) out[c] = (hi + lo) * g.vol;
-}
-
-// ---- FP64 pipe probe (measurement only: the second roofline of DESIGN.md sec. 5) ----------
-// MODE 0: 8 independent DFMA chains per thread; MODE 1: the same with DADD/DMUL alternating (no
-// FMA); MODE 2: every DFMA followed by one independent integer multiply-add, to see whether the
-// other pipes issue under a busy FP64 pipe or wait for it.  out[] keeps the results alive.
-template <int MODE>
-__global__ void __launch_bounds__(256)
-k_fp64_probe(double* out, int iters, double c0, double c1)
-{
-    double x[8];
-    unsigned k[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { x[q] = c0 + (double)(threadIdx.x + q); k[q] = threadIdx.x * 8u + q; }
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            if (MODE == 1) x[q] = (it & 1) ? __dmul_rn(x[q], c1) : __dadd_rn(x[q], c0);
-            else x[q] = fma(x[q], c1, c0);
-            if (MODE == 2) k[q] = k[q] * 1664525u + (unsigned)it;
-        }
-    }
-    double s = 0.0;
-    unsigned ks = 0;
-#pragma unroll
-    for (int q = 0; q < 8; ++q) { s += x[q]; ks += k[q]; }
-    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s + (double)(ks & 1u);
 }
 
 }  // namespace hydro

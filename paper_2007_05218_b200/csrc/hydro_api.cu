@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -16,6 +17,7 @@
 #include "sweep_x.cuh"
 #include "sweep_yz.cuh"
 #include "march_ring.cuh"
+#include "march_x.cuh"
 
 using namespace hydro;
 
@@ -29,11 +31,47 @@ constexpr int BS = 128;               // threads per CTA of the marching kernels
 #define HYDRO_RING_D 8
 #endif
 constexpr int RING_D = HYDRO_RING_D;  // depth of the TMA ring of the marching kernels
+#ifndef HYDRO_XM_D
+#define HYDRO_XM_D 3
+#endif
+constexpr int XM_D = HYDRO_XM_D;      // depth of the ring of the x marching kernels (a step is four zones)
+#ifndef HYDRO_XS_MODE
+#define HYDRO_XS_MODE 1               // x species kernels: 1 = one species per thread, one thread set per species of the
+#endif                                // group; 0 = one thread per row marches the whole group
+#ifndef HYDRO_XS_ROWS
+#define HYDRO_XS_ROWS 32
+#endif
+constexpr int XS_ROWS = HYDRO_XS_MODE ? HYDRO_XS_ROWS : XBS;   // rows per CTA of the x species kernels
+
+constexpr int DT_SLOTS = 1024;        // (dt, max t) pairs kept on the device: one per step of a hydro_step chunk
+constexpr int PROF_EVENTS = 8192;     // event pool of hydro_profile (two per recorded launch)
 
 thread_local std::string g_init_error = "";
 
 struct Carve {
     size_t lacc, frho, part, totals, red, dtslot, flat, zc, total;
+};
+
+// tuning switches, read from the environment ONCE per hydro_init (include/hydro.h lists them)
+struct Knobs {
+    int ring, seglen, nsmax, fuse_dt, split_ghosts, fill_monolithic, xmarch;
+};
+
+int env_int(const char *name, int dflt)
+{
+    const char *e = getenv(name);
+    return (e && *e) ? atoi(e) : dflt;
+}
+
+// makes the handle's device current for the duration of an entry point
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
 }  // namespace
@@ -45,8 +83,11 @@ struct hydro_ctx {
     char *scratch;
     Carve cv;
     cudaStream_t stream;
-    double *pinned;           // nflux + 2 doubles of pinned host memory
+    int device;               // the device the caller's buffers live on; made current by every entry point
+    double *pinned;           // max(nflux, 2 * DT_SLOTS) doubles of pinned host memory
     long long launches;
+    Knobs kn;
+    std::set<const void *> configured;   // kernels whose dynamic shared-memory limit is set on `device`
     int seglen[3];
     int ns_max;
     bool use_ring;            // TMA-ring marching kernels usable for this geometry
@@ -54,12 +95,18 @@ struct hydro_ctx {
     bool fuse_dt;             // hydro_step: the stage-1 z hydro sweep also reduces the next step's dt
     CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
     CUtensorMap fmaps[2];      // [DIR-1]: TMA views of the flattening-coefficient array (flatten == 1)
+    bool use_xmarch;           // x sweep by the marching kernels of march_x.cuh (else k_sweep_x)
+    CUtensorMap xmaps[2][6];   // [state][components per box]: {4 zones, 128 rows} views for the x hydro marching kernel
+    CUtensorMap xsmaps[2][6];  // the same with XS_ROWS rows per box, for the x species marching kernels
     std::string err;
-    // optional per-launch timing (hydro_profile): event pairs on the handle's stream
+    // optional per-launch timing (hydro_profile): event pairs from a pool created by hydro_profile(1);
+    // nothing is allocated while launches are recorded (when the pool is used up, recording stops)
     bool profiling;
-    struct Ev { cudaEvent_t a, b; int klass; };
+    std::vector<cudaEvent_t> pool;
+    size_t pool_used;
+    struct Ev { int a, b, klass; };
     std::vector<Ev> events;
-    cudaEvent_t pending;
+    int pending;
 };
 
 namespace {
@@ -100,15 +147,19 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
         g.dxinv[d] = 1.0 / dx[d];
         g.grav[d] = p->grav[d];
     }
-    if (g.nboxes > 65535) { why = "more than 65535 boxes"; return false; }
+    if (g.nboxes > (1 << 20)) { why = "more than 2^20 boxes"; return false; }
     g.cstride = (long long)g.nt[0] * g.nt[1] * g.nt[2];
     g.bstride = g.cstride * g.nvar;
     g.lcstride = (long long)g.nb[0] * g.nb[1] * g.nb[2];
     // accumulator components per zone: the NFLUX flux differences; with O11 three more (flux of rho*e,
     // div(u_face), rho*E - K of the new state)
     g.lbstride = g.lcstride * (g.nflux + (p->evolve_eint ? 3 : 0));
+    // one face mass-flux array serves the three sweeps in turn: y and z faces as (nb+1)-extended arrays, x faces
+    // in rows of nb0 + 4 (march_x.cuh)
     g.fbstride = (long long)(g.nb[0] + 1) * (g.nb[1] + 1) * (g.nb[2] + 1);
-    g.fbstride += g.fbstride & 1;                     // keep every box's face array 16-byte aligned
+    const long long fx = (long long)(g.nb[0] + 4) * g.nb[1] * g.nb[2];
+    if (fx > g.fbstride) g.fbstride = fx;
+    g.fbstride = (g.fbstride + 3) & ~3LL;             // keep every box's face array 32-byte aligned
     g.gamma = p->gamma; g.gm1 = p->gamma - 1.0; g.gm1inv = 1.0 / (p->gamma - 1.0);
     g.small_dens = p->small_dens; g.small_pres = p->small_pres;
     g.floor_rhoe = p->small_pres * g.gm1inv;
@@ -129,7 +180,7 @@ Carve carve(const Geom &g)
     c.part = off;   off += up256((size_t)g.nflux * RED_BLOCKS * 2 * 8);
     c.totals = off; off += up256((size_t)g.nflux * 8);
     c.red = off;    off += 256;
-    c.dtslot = off; off += 256;
+    c.dtslot = off; off += up256((size_t)DT_SLOTS * 16);
     c.flat = off;   if (g.flatten) off += up256((size_t)g.cstride * g.nboxes * 8);   // O10 coefficients
     c.zc = off;     if (g.flatten) off += up256((size_t)g.cstride * g.nboxes * 3 * 8); // O10 chi*z per direction
     c.total = off;
@@ -170,6 +221,35 @@ bool make_ring_map(CUtensorMap *out, double *U, const Geom &g, int dir, int nc, 
     return true;
 }
 
+// TMA view of one state for the x marching kernels: the same 5-D tensor with a box of XC zones x RJ rows (j) x
+// RK rows (k) x nc components; thread t of the CTA reads row t of the box.
+bool make_xmarch_map(CUtensorMap *out, double *U, const Geom &g, int nc, int rows, std::string &why)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+        why = "cuTensorMapEncodeTiled is not available from the driver";
+        return false;
+    }
+    const int RJ = g.nb[1] < rows ? g.nb[1] : rows, RK = rows / RJ;
+    cuuint64_t dims[5] = {(cuuint64_t)g.nt[0], (cuuint64_t)g.nt[1], (cuuint64_t)g.nt[2], (cuuint64_t)g.nvar,
+                          (cuuint64_t)g.nboxes};
+    cuuint64_t strides[4] = {(cuuint64_t)g.nt[0] * 8, (cuuint64_t)g.nt[0] * g.nt[1] * 8, (cuuint64_t)g.cstride * 8,
+                             (cuuint64_t)g.bstride * 8};
+    cuuint32_t box[5] = {(cuuint32_t)XC, (cuuint32_t)RJ, (cuuint32_t)RK, (cuuint32_t)nc, 1u};
+    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+#ifndef HYDRO_XM_PROMO
+#define HYDRO_XM_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
+    CUresult r = ((encode_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 CU_TENSOR_MAP_SWIZZLE_NONE, HYDRO_XM_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
 int fail(hydro_handle h, int code, const std::string &msg)
 {
     if (h) h->err = msg; else g_init_error = msg;
@@ -181,30 +261,31 @@ enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIE
 
 void prof_begin(hydro_handle h)
 {
-    if (!h->profiling) return;
-    cudaEventCreate(&h->pending);
-    cudaEventRecord(h->pending, h->stream);
+    h->pending = -1;
+    if (!h->profiling || h->pool_used + 2 > h->pool.size()) return;
+    h->pending = (int)h->pool_used;
+    cudaEventRecord(h->pool[h->pending], h->stream);
 }
 
 int check_launch(hydro_handle h, const char *what, int klass)
 {
     cudaError_t e = cudaGetLastError();
     h->launches++;
-    if (h->profiling && e == cudaSuccess) {
+    if (h->profiling && h->pending >= 0 && e == cudaSuccess) {
         hydro_ctx::Ev ev;
-        ev.a = h->pending; ev.klass = klass;
-        cudaEventCreate(&ev.b);
-        cudaEventRecord(ev.b, h->stream);
-        h->events.push_back(ev);
+        ev.a = h->pending; ev.b = h->pending + 1; ev.klass = klass;
+        cudaEventRecord(h->pool[ev.b], h->stream);
+        h->pool_used += 2;
+        h->events.push_back(ev);          // capacity reserved by hydro_profile(1)
     }
+    h->pending = -1;
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
     return HYDRO_OK;
 }
 
-int pick_seglen(const Geom &g, int dir)
+int pick_seglen(const Geom &g, int dir, int forced)
 {
-    const char *env = getenv("HYDRO_SEGLEN");
-    if (env && atoi(env) > 0) return atoi(env) < g.nb[dir] ? atoi(env) : g.nb[dir];
+    if (forced > 0) return forced < g.nb[dir] ? forced : g.nb[dir];
     // enough pencils to fill 148 SMs several times over? then march the whole box
     const int T = dir == 1 ? 2 : 1;
     long long pencils = (long long)g.nb[0] * g.nb[T] * g.nboxes;
@@ -213,10 +294,14 @@ int pick_seglen(const Geom &g, int dir)
     return (g.nb[dir] + nseg - 1) / nseg;
 }
 
+// The ring kernels need more than the default 48 KB of dynamic shared memory.  The limit is a per-device
+// attribute of a kernel, so it is set once per (handle, kernel): a handle lives on one device.
 template <typename K>
-void set_smem(K kernel, size_t bytes)
+void set_smem(hydro_handle h, K kernel, size_t bytes)
 {
+    if (h->configured.count((const void *)kernel)) return;
     cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    h->configured.insert((const void *)kernel);
 }
 
 template <int DIR, bool FINAL, int STAGE, int N, bool FLAT>
@@ -224,7 +309,7 @@ void launch_species_ring_n(hydro_handle h, const SweepArgs &a, dim3 grid, const 
 {
     const size_t sm = (size_t)RING_D * (1 + N + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
     auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D, FLAT>;
-    static bool once = (set_smem(kern, sm), true); (void)once;
+    set_smem(h, kern, sm);
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
 
@@ -233,7 +318,7 @@ void launch_energy_ring(hydro_handle h, const SweepArgs &a, dim3 grid, const Rin
 {
     const size_t sm = (size_t)RING_D * (2 + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
     auto kern = k_march_species<DIR, FINAL, STAGE, 1, BS, RING_D, FLAT, FINAL>;   // ENERGY terms only in the FINAL sweep
-    static bool once = (set_smem(kern, sm), true); (void)once;
+    set_smem(h, kern, sm);
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
 
@@ -262,7 +347,7 @@ void launch_hydro_ring(hydro_handle h, const SweepArgs &a, dim3 grid, int state)
     constexpr int NROW = (FINAL ? 6 : 5) + (FLAT ? 1 : 0);
     const size_t sm = (size_t)RING_D * NROW * BS * 8 + RING_D * 8;
     auto kern = k_march_hydro<DIR, FINAL, STAGE, BS, RING_D, FLAT, EVOLVE>;
-    static bool once = (set_smem(kern, sm), true); (void)once;
+    set_smem(h, kern, sm);
     RingMaps tm;
     tm.a = h->maps[state][DIR - 1][FINAL ? 6 : 4];
     tm.b = h->maps[state][DIR - 1][1];
@@ -288,12 +373,14 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     constexpr int T = DIR == 1 ? 2 : 1;
     a.seglen = h->seglen[DIR];
     const int nseg = (g.nb[DIR] + a.seglen - 1) / a.seglen;
-    dim3 grid((g.nb[0] * g.nb[T] + BS - 1) / BS, nseg, g.nboxes);
+    dim3 grid((g.nb[0] * g.nb[T] + BS - 1) / BS, nseg, 1);
     const bool ring = h->use_ring;
     if (ring) {   // CTA = R row segments of W zones; rows may not fill the last CTA
         const int W = g.nb[0] < BS ? g.nb[0] : BS, R = BS / W;
         grid.x = (g.nb[T] * (g.nb[0] / W) + R - 1) / R;
     }
+    if ((long long)grid.x * g.nboxes > 2147483647LL || nseg > 65535) return fail(h, HYDRO_EINVAL, "sweep grid too large");
+    grid.x *= g.nboxes;   // the box index rides in blockIdx.x
     prof_begin(h);
     if (ring) {
         if (g.flatten && g.evolve) launch_hydro_ring<DIR, FINAL, STAGE, true, true>(h, a, grid, state);
@@ -334,6 +421,72 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     return HYDRO_OK;
 }
 
+template <int N>
+void launch_xmarch_species_n(hydro_handle h, const XArgs &xa, dim3 grid, const XMaps &tm)
+{
+    const size_t sm = (size_t)XM_D * (1 + N) * XS_ROWS * XC * 8 + XM_D * 8;
+#if HYDRO_XS_MODE
+    auto kern = k_xmarch_species<1, N, XS_ROWS, XM_D>;
+    const int threads = XS_ROWS * N;
+#else
+    auto kern = k_xmarch_species<N, 1, XS_ROWS, XM_D>;
+    const int threads = XS_ROWS;
+#endif
+    set_smem(h, kern, sm);
+    kern<<<grid, threads, sm, h->stream>>>(h->g, xa, tm);
+}
+
+// x sweep of a stage by the marching kernels: hydro launch (writes the accumulator rows of the five hydro
+// variables and F_rho,x), then one species launch per group
+int xmarch_stage(hydro_handle h, int state, double *Lacc, double *FX)
+{
+    const Geom &g = h->g;
+    const int RJ = g.nb[1] < XBS ? g.nb[1] : XBS, RK = XBS / RJ;
+    const long long tiles = (long long)(g.nb[1] / RJ) * ((g.nb[2] + RK - 1) / RK);
+    if (tiles * g.nboxes > 2147483647LL) return fail(h, HYDRO_EINVAL, "x-march grid too large");
+    const dim3 grid((unsigned)(tiles * g.nboxes), 1, 1);
+    XArgs xa;
+    xa.Lacc = Lacc; xa.FX = FX; xa.sbase = 0;
+    XMaps tm;
+    {
+        const size_t sm = (size_t)XM_D * 5 * XBS * XC * 8 + XM_D * 8;
+        auto kern = k_xmarch_hydro<XM_D>;
+        set_smem(h, kern, sm);
+        tm.a = h->xmaps[state][4];
+        tm.b = h->xmaps[state][1];
+        prof_begin(h);
+        kern<<<grid, XBS, sm, h->stream>>>(g, xa, tm);
+        int rc = check_launch(h, "k_xmarch_hydro", K_SWEEP_X);
+        if (rc) return rc;
+    }
+    if (g.nspec > 0) {
+        const int SJ = g.nb[1] < XS_ROWS ? g.nb[1] : XS_ROWS, SK = XS_ROWS / SJ;
+        const dim3 sgrid((unsigned)((long long)(g.nb[1] / SJ) * ((g.nb[2] + SK - 1) / SK) * g.nboxes), 1, 1);
+        const int ngroups = (g.nspec + h->ns_max - 1) / h->ns_max;
+        const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
+        int s0 = 0;
+        for (int gr = 0; gr < ngroups; ++gr) {
+            const int ns = base + (gr < rem ? 1 : 0);
+            xa.sbase = s0;
+            tm.a = h->xsmaps[state][1];
+            tm.b = h->xsmaps[state][ns];
+            prof_begin(h);
+            switch (ns) {
+                case 1: launch_xmarch_species_n<1>(h, xa, sgrid, tm); break;
+                case 2: launch_xmarch_species_n<2>(h, xa, sgrid, tm); break;
+                case 3: launch_xmarch_species_n<3>(h, xa, sgrid, tm); break;
+                case 4: launch_xmarch_species_n<4>(h, xa, sgrid, tm); break;
+                case 5: launch_xmarch_species_n<5>(h, xa, sgrid, tm); break;
+                default: break;
+            }
+            int rc = check_launch(h, "k_xmarch_species", K_SWEEP_X);
+            if (rc) return rc;
+            s0 += ns;
+        }
+    }
+    return HYDRO_OK;
+}
+
 int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_dev, bool xends = false,
                        double *dt_next = nullptr)
 {
@@ -354,9 +507,12 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     if (g.flatten) {   // O10: flattening coefficients of the stage state (ghosts are filled) before any sweep
         a.FL = (const double *)(h->scratch + h->cv.flat);
         auto fgrid = [&](int lo) {
-            return dim3((g.nb[0] - 2 * lo + FLT_BX - 1) / FLT_BX, (g.nb[1] - 2 * lo + FLT_BY - 1) / FLT_BY,
-                        (unsigned)(((g.nb[2] - 2 * lo + FLT_BZ - 1) / FLT_BZ) * g.nboxes));
+            return dim3((unsigned)(((g.nb[0] - 2 * lo + FLT_BX - 1) / FLT_BX) * g.nboxes), (g.nb[1] - 2 * lo + FLT_BY - 1) / FLT_BY,
+                        (g.nb[2] - 2 * lo + FLT_BZ - 1) / FLT_BZ);
         };
+        if ((long long)((g.nb[0] + 4 + FLT_BX - 1) / FLT_BX) * g.nboxes > 2147483647LL || g.nb[1] + 4 > 65535 * FLT_BY ||
+            g.nb[2] + 4 > 65535 * FLT_BZ)
+            return fail(h, HYDRO_EINVAL, "flattening grid too large");
         double *ZC = (double *)(h->scratch + h->cv.zc);
         prof_begin(h);
         k_flatten_zc<<<fgrid(-2), dim3(FLT_BX, FLT_BY, FLT_BZ), 0, h->stream>>>(g, a.Us, ZC);
@@ -367,13 +523,16 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
         int rc = check_launch(h, "k_flatten", K_FLATTEN);
         if (rc) return rc;
     }
-    {   // x sweep: one warp per 26-zone chunk of a row
+    if (h->use_xmarch) {   // x sweep: a thread per row, marching (march_x.cuh)
+        int rc = xmarch_stage(h, stage, a.Lacc, a.Frho);
+        if (rc) return rc;
+    } else {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
-        const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS);
+        const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS) * g.nboxes;
         if (gx > 2147483647LL || g.nb[2] > 65535) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
         prof_begin(h);
-        const dim3 xg((unsigned)gx, g.nb[2], g.nboxes);
+        const dim3 xg((unsigned)gx, g.nb[2], 1);
         if (g.flatten && g.evolve) k_sweep_x<WARPS, true, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
         else if (g.flatten) k_sweep_x<WARPS, true, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
         else if (g.evolve) k_sweep_x<WARPS, false, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
@@ -392,19 +551,19 @@ int fill_ghost_rows_impl(hydro_handle h, int which);
 int fill_ghosts_impl(hydro_handle h, int which)
 {
     const Geom &g = h->g;
-    if (g.nvar > 65535) return fail(h, HYDRO_EINVAL, "too many components for the ghost grid");
-    const char *em = getenv("HYDRO_FILL_MONOLITHIC");
-    if (h->split_ghosts && (long long)g.nvar * g.nboxes <= 65535 && g.nb[2] <= 65535 && !(em && atoi(em) != 0)) {
+    if (g.nvar > 65535 || (long long)g.nt[2] * g.nboxes > 2147483647LL)
+        return fail(h, HYDRO_EINVAL, "ghost-fill grid too large");
+    if (h->split_ghosts && g.nb[2] <= 65535 && !h->kn.fill_monolithic) {
         // split form (bit-identical, less index arithmetic and no 32-byte row-end gathers in the plane
         // kernel): x ghost zones of the valid rows, then the ghost rows as whole-row copies
         prof_begin(h);
-        k_fill_xends<<<dim3((g.nb[1] * 2 * g.ng + 255) / 256, g.nb[2], g.nvar * g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
+        k_fill_xends<<<dim3((unsigned)(((g.nb[1] * 2 * g.ng + 255) / 256) * g.nboxes), g.nb[2], g.nvar), 256, 0, h->stream>>>(g, h->U[which]);
         int rc = check_launch(h, "k_fill_xends", K_GHOST);
         if (rc) return rc;
         return fill_ghost_rows_impl(h, which);
     }
     prof_begin(h);
-    k_fill_ghosts<<<dim3(g.nt[2], g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
+    k_fill_ghosts<<<dim3((unsigned)(g.nt[2] * g.nboxes), g.nvar, 1), 256, 0, h->stream>>>(g, h->U[which]);
     return check_launch(h, "k_fill_ghosts", K_GHOST);
 }
 
@@ -414,13 +573,14 @@ int fill_ghost_rows_impl(hydro_handle h, int which)
     const Geom &g = h->g;
     const int nrows = g.nt[2] * g.nt[1] - g.nb[2] * g.nb[1];
     prof_begin(h);
-    k_fill_ghost_rows<<<dim3((nrows + GR_ROWS - 1) / GR_ROWS, g.nvar, g.nboxes), 256, 0, h->stream>>>(g, h->U[which]);
+    k_fill_ghost_rows<<<dim3((unsigned)(((nrows + GR_ROWS - 1) / GR_ROWS) * g.nboxes), g.nvar, 1), 256, 0, h->stream>>>(g, h->U[which]);
     return check_launch(h, "k_fill_ghost_rows", K_GHOST);
 }
 
-// two dt slots of (dt, max t): hydro_step alternates them so that the dt of step s+1, reduced by
-// the last hydro kernel of step s, does not overwrite the dt the rest of step s still reads
-double *dt_slot(hydro_handle h, int slot) { return (double *)(h->scratch + h->cv.dtslot) + 2 * slot; }
+// (dt, max t) slots on the device, one per step of a hydro_step chunk: the dt of step s+1, reduced by the
+// last hydro kernel of step s, must not overwrite the dt the rest of step s still reads, and the host
+// validates every step's max t after the chunk
+double *dt_slot(hydro_handle h, int slot) { return (double *)(h->scratch + h->cv.dtslot) + 2 * (slot % DT_SLOTS); }
 
 int launch_dt(hydro_handle h, int slot = 0)
 {
@@ -434,61 +594,43 @@ int launch_dt(hydro_handle h, int slot = 0)
     return check_launch(h, "k_estimate_dt", K_DT);
 }
 
-int read_dt(hydro_handle h, double *dt_host, int slot = 0)
+// read back slots 0..n-1, validate every max t, copy the dts to dt_host (may be NULL)
+int read_dts(hydro_handle h, double *dt_host, int n)
 {
-    cudaError_t e = cudaMemcpyAsync(h->pinned, dt_slot(h, slot), 16, cudaMemcpyDeviceToHost, h->stream);
+    cudaError_t e = cudaMemcpyAsync(h->pinned, dt_slot(h, 0), (size_t)n * 16, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("dt read-back: ") + cudaGetErrorString(e));
-    const double dt = h->pinned[0], tmax = h->pinned[1];
-    if (!(tmax > 0.0) || !std::isfinite(tmax) || !std::isfinite(dt))
-        return fail(h, HYDRO_ESTATE, "estimate_dt: max signal speed is not a positive finite number");
-    *dt_host = dt;
-    return HYDRO_OK;
-}
-
-}  // namespace
-
-namespace {
-template <int C, int D>
-int tma_probe_run(int nc, double *buf, long long rows, double *out, double *gbs)
-{
-    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
-                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    void *fn = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn)
-        return fail(nullptr, HYDRO_ECUDA, "cuTensorMapEncodeTiled is not available from the driver");
-    const int pitch = 136, ncols = 128;
-    CUtensorMap tm;
-    cuuint64_t dims[3] = {(cuuint64_t)pitch, (cuuint64_t)rows, (cuuint64_t)nc};
-    cuuint64_t strides[2] = {(cuuint64_t)pitch * 8, (cuuint64_t)pitch * rows * 8};
-    cuuint32_t box[3] = {C, 128, 1}, estr[3] = {1, 1, 1};
-    if (((encode_fn)fn)(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, buf, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return fail(nullptr, HYDRO_ECUDA, "hydro_tma_probe: cuTensorMapEncodeTiled failed");
-    const size_t sm = (size_t)D * nc * 128 * C * 8 + D * 8;
-    if (sm > 220 * 1024) return fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: ring does not fit in shared memory");
-    cudaFuncSetAttribute(k_tma_probe<C, D>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
-        cudaEventRecord(e0);
-        k_tma_probe<C, D><<<(unsigned)(rows / 128), 128, sm>>>(tm, nc, ncols, out);
-        cudaEventRecord(e1);
-        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
-            cudaEventDestroy(e0); cudaEventDestroy(e1);
-            return fail(nullptr, HYDRO_ECUDA, "hydro_tma_probe: kernel failed");
-        }
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best) best = ms;
+    for (int s = 0; s < n; ++s) {
+        const double dt = h->pinned[2 * s], tmax = h->pinned[2 * s + 1];
+        if (!(tmax > 0.0) || !std::isfinite(tmax) || !std::isfinite(dt))
+            return fail(h, HYDRO_ESTATE, "estimate_dt: max signal speed is not a positive finite number (step " +
+                                             std::to_string(s) + " of the call)");
+        if (dt_host) dt_host[s] = dt;
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    *gbs = (double)rows * ncols * 8 * nc / (best * 1e-3) / 1e9;
     return HYDRO_OK;
 }
+
+// one chunk of at most DT_SLOTS steps; step s of the chunk keeps its (dt, max t) in slot s
+int step_chunk(hydro_handle h, int nsteps, double *dt_host)
+{
+    int rc;
+    const bool split = h->split_ghosts, fuse = h->fuse_dt;
+    for (int s = 0; s < nsteps; ++s) {
+        const double *dt_dev = dt_slot(h, s);
+        // the caller's U0 gets the dt kernel; later steps use the dt that the stage-1 z sweep of the
+        // previous step reduced from the very values it wrote (same formula, same bits)
+        if (s == 0 || !fuse) if ((rc = launch_dt(h, s))) return rc;
+        // the caller's U0 gets the full fill; after that stage 1 has left every valid row of U0
+        // complete (x images written by the z sweeps) and only the ghost rows remain
+        if ((rc = (split && s > 0) ? fill_ghost_rows_impl(h, 0) : fill_ghosts_impl(h, 0))) return rc;
+        if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev, split))) return rc;
+        if ((rc = split ? fill_ghost_rows_impl(h, 1) : fill_ghosts_impl(h, 1))) return rc;
+        double *dt_next = (fuse && s + 1 < nsteps) ? dt_slot(h, s + 1) : nullptr;
+        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split, dt_next))) return rc;
+    }
+    return read_dts(h, dt_host, nsteps);
+}
+
 }  // namespace
 
 extern "C" {
@@ -520,19 +662,42 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     if (U0_dev == U1_dev) return fail(nullptr, HYDRO_EINVAL, "U0 and U1 must be distinct");
     Carve cv = carve(g);
     if (scratch_bytes < cv.total) return fail(nullptr, HYDRO_ENOMEM, "scratch_bytes too small");
+    // the device of the handle = the device the caller's buffers live on (all three on the same one)
+    int device = -1;
+    {
+        void *bufs[3] = {U0_dev, U1_dev, scratch_dev};
+        for (void *b : bufs) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, b) != cudaSuccess || at.type != cudaMemoryTypeDevice) {
+                cudaGetLastError();
+                return fail(nullptr, HYDRO_EINVAL, "U0_dev, U1_dev and scratch_dev must be device memory");
+            }
+            if (device >= 0 && at.device != device)
+                return fail(nullptr, HYDRO_EINVAL, "U0_dev, U1_dev and scratch_dev must live on one device");
+            device = at.device;
+        }
+    }
+    DeviceGuard guard(device);
     hydro_ctx *h = new (std::nothrow) hydro_ctx();
     if (!h) return fail(nullptr, HYDRO_ENOMEM, "host allocation failed");
     h->p = *p; h->g = g; h->U[0] = (double *)U0_dev; h->U[1] = (double *)U1_dev;
     h->scratch = (char *)scratch_dev; h->cv = cv; h->stream = (cudaStream_t)cuda_stream;
-    h->launches = 0; h->pinned = nullptr; h->profiling = false;
-    const char *env = getenv("HYDRO_NSMAX");
-    h->ns_max = (env && atoi(env) >= 1 && atoi(env) <= NS_MAX) ? atoi(env) : NS_MAX;
-    for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d);
+    h->device = device;
+    h->launches = 0; h->pinned = nullptr; h->profiling = false; h->pool_used = 0; h->pending = -1;
+    // tuning switches (include/hydro.h): read here, once
+    h->kn.ring = env_int("HYDRO_RING", 1);
+    h->kn.seglen = env_int("HYDRO_SEGLEN", 0);
+    h->kn.nsmax = env_int("HYDRO_NSMAX", NS_MAX);
+    h->kn.fuse_dt = env_int("HYDRO_FUSE_DT", 1);
+    h->kn.split_ghosts = env_int("HYDRO_SPLIT_GHOSTS", 1);
+    h->kn.fill_monolithic = env_int("HYDRO_FILL_MONOLITHIC", 0);
+    h->kn.xmarch = env_int("HYDRO_XMARCH", 0);
+    h->ns_max = (h->kn.nsmax >= 1 && h->kn.nsmax <= NS_MAX) ? h->kn.nsmax : NS_MAX;
+    for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d, h->kn.seglen);
     {   // TMA tensor copies: 16-byte row pitch AND 16-byte aligned box starts (the first valid zone of a row sits
         // ng doubles in, so ng must be even), row segments that tile the CTA exactly
         const int W = g.nb[0] < BS ? g.nb[0] : BS;
-        const char *er = getenv("HYDRO_RING");
-        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && !(er && atoi(er) == 0);
+        h->use_ring = (g.ng % 2 == 0) && (g.nb[0] % 2 == 0) && (BS % W == 0) && (g.nb[0] % W == 0) && h->kn.ring != 0;
         for (int st = 0; st < 2 && h->use_ring; ++st)
             for (int dir = 1; dir <= 2 && h->use_ring; ++dir)
                 for (int nc = 1; nc <= 6 && h->use_ring; ++nc) {
@@ -541,9 +706,25 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
                     if (!make_ring_map(&h->maps[st][dir - 1][nc], h->U[st], g, dir, nc, why2)) h->use_ring = false;
                 }
     }
+    {   // x marching kernels: rows of nb0 in whole 4-zone steps, 128 rows per CTA, zones -4 .. nb0+3 inside the padded
+        // row at 16-byte aligned starts; the options O10 / O11 stay with k_sweep_x
+        h->use_xmarch = h->kn.xmarch != 0 && g.ng % 2 == 0 && g.ng >= 4 && g.nb[0] % XC == 0 &&
+                        (XBS % g.nb[1] == 0 || g.nb[1] % XBS == 0) && (XS_ROWS % g.nb[1] == 0 || g.nb[1] % XS_ROWS == 0) &&
+                        !g.flatten && !g.evolve;
+        for (int st = 0; st < 2 && h->use_xmarch; ++st)
+            for (int nc = 1; nc <= 5 && h->use_xmarch; ++nc) {
+                if (nc > g.nvar) continue;
+                std::string why2;
+                if (!make_xmarch_map(&h->xmaps[st][nc], h->U[st], g, nc, XBS, why2)) h->use_xmarch = false;
+                if (!make_xmarch_map(&h->xsmaps[st][nc], h->U[st], g, nc, XS_ROWS, why2)) h->use_xmarch = false;
+            }
+    }
+    cudaError_t e = cudaSuccess;
     if (g.flatten) {   // coefficient array = 1 (no flattening) outside the zones k_flatten writes
         double *FL = (double *)(h->scratch + cv.flat);
         k_fill_value<<<148 * 8, 256, 0, h->stream>>>(FL, (long long)g.cstride * g.nboxes, 1.0);
+        e = cudaGetLastError();
+        h->launches++;
         for (int dir = 1; dir <= 2 && h->use_ring; ++dir) {
             std::string why2;
             if (!make_ring_map(&h->fmaps[dir - 1], FL, g, dir, 1, why2, 1, g.cstride)) h->use_ring = false;
@@ -554,15 +735,13 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
         return fail(nullptr, HYDRO_EINVAL, "evolve_eint = 1 needs a geometry the TMA-ring kernels accept "
                                            "(even ng, even nbox[0] that divides or is a multiple of 128)");
     }
-    {   // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
-        const char *ed = getenv("HYDRO_FUSE_DT");
-        h->fuse_dt = h->use_ring && !g.evolve && !(ed && atoi(ed) == 0);   // O11: rho*e is final only after the energy kernel
-        const char *ef = getenv("HYDRO_SPLIT_GHOSTS");
-        h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng &&
-                          g.nb[2] >= g.ng && !(ef && atoi(ef) == 0);
-    }
-    cudaError_t e = cudaMallocHost((void **)&h->pinned, (size_t)(g.nflux + 2) * 8);
-    if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 512, h->stream);
+    // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
+    h->fuse_dt = h->use_ring && !g.evolve && h->kn.fuse_dt != 0;   // O11: rho*e is final only after the energy kernel
+    h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng && g.nb[2] >= g.ng &&
+                      h->kn.split_ghosts != 0;
+    const size_t npin = (size_t)(g.nflux > 2 * DT_SLOTS ? g.nflux : 2 * DT_SLOTS);
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&h->pinned, npin * 8);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 256, h->stream);
     if (e != cudaSuccess) {
         std::string msg = std::string("hydro_init: ") + cudaGetErrorString(e);
         if (h->pinned) cudaFreeHost(h->pinned);
@@ -577,6 +756,7 @@ int hydro_fill_ghosts(hydro_handle h, int which)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (which != 0 && which != 1) return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
+    DeviceGuard guard(h->device);
     return fill_ghosts_impl(h, which);
 }
 
@@ -584,6 +764,7 @@ int hydro_advance_stage(hydro_handle h, int stage, double dt)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (stage != 0 && stage != 1) return fail(h, HYDRO_EINVAL, "stage must be 0 or 1");
+    DeviceGuard guard(h->device);
     return advance_stage_impl(h, stage, dt, nullptr);
 }
 
@@ -591,9 +772,10 @@ int hydro_estimate_dt(hydro_handle h, double *dt_host)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (!dt_host) return fail(h, HYDRO_EINVAL, "null dt_host");
+    DeviceGuard guard(h->device);
     int rc = launch_dt(h);
     if (rc) return rc;
-    return read_dt(h, dt_host);
+    return read_dts(h, dt_host, 1);
 }
 
 int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
@@ -601,6 +783,7 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (which != 0 && which != 1) return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
     if (!totals_host) return fail(h, HYDRO_EINVAL, "null totals_host");
+    DeviceGuard guard(h->device);
     const Geom &g = h->g;
     const long long nrows = (long long)g.nb[1] * g.nb[2] * g.nboxes;
     long long blocks = (nrows + 7) / 8;            // 8 warps per block, one row per warp and trip
@@ -621,27 +804,16 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host)
     return HYDRO_OK;
 }
 
-int hydro_step(hydro_handle h, int nsteps, double *dt_last_host)
+int hydro_step(hydro_handle h, int nsteps, double *dt_host)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
-    int rc;
-    const bool split = h->split_ghosts, fuse = h->fuse_dt;
-    for (int s = 0; s < nsteps; ++s) {
-        const int slot = s & 1;
-        const double *dt_dev = dt_slot(h, slot);
-        // the caller's U0 gets the dt kernel; later steps use the dt that the stage-1 z sweep of the
-        // previous step reduced from the very values it wrote (same formula, same bits)
-        if (s == 0 || !fuse) if ((rc = launch_dt(h, slot))) return rc;
-        // the caller's U0 gets the full fill; after that stage 1 has left every valid row of U0
-        // complete (x images written by the z sweeps) and only the ghost rows remain
-        if ((rc = (split && s > 0) ? fill_ghost_rows_impl(h, 0) : fill_ghosts_impl(h, 0))) return rc;
-        if ((rc = advance_stage_impl(h, 0, 0.0, dt_dev, split))) return rc;
-        if ((rc = split ? fill_ghost_rows_impl(h, 1) : fill_ghosts_impl(h, 1))) return rc;
-        double *dt_next = (fuse && s + 1 < nsteps) ? dt_slot(h, (s + 1) & 1) : nullptr;
-        if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split, dt_next))) return rc;
+    DeviceGuard guard(h->device);
+    for (int done = 0; done < nsteps; done += DT_SLOTS) {
+        const int n = nsteps - done < DT_SLOTS ? nsteps - done : DT_SLOTS;
+        int rc = step_chunk(h, n, dt_host ? dt_host + done : nullptr);
+        if (rc) return rc;
     }
-    if (dt_last_host && nsteps > 0) return read_dt(h, dt_last_host, (nsteps - 1) & 1);
     return HYDRO_OK;
 }
 
@@ -653,6 +825,7 @@ int hydro_query(hydro_handle h, int what)
         case 1: return h->split_ghosts ? 1 : 0;
         case 2: return h->fuse_dt ? 1 : 0;
         case 3: return h->ns_max;
+        case 4: return h->use_xmarch ? 1 : 0;
         default: return -1;
     }
 }
@@ -662,6 +835,16 @@ long long hydro_launch_count(hydro_handle h) { return h ? h->launches : 0; }
 int hydro_profile(hydro_handle h, int enable)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    DeviceGuard guard(h->device);
+    if (enable && h->pool.empty()) {      // the event pool is created here, never while launches are recorded
+        h->pool.resize(PROF_EVENTS);
+        for (auto &ev : h->pool)
+            if (cudaEventCreate(&ev) != cudaSuccess) {
+                h->pool.clear();
+                return fail(h, HYDRO_ECUDA, "hydro_profile: cudaEventCreate failed");
+            }
+        h->events.reserve(PROF_EVENTS / 2);
+    }
     h->profiling = enable != 0;
     return HYDRO_OK;
 }
@@ -670,81 +853,31 @@ int hydro_profile_read(hydro_handle h, double *ms_host, long long *count_host)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (!ms_host || !count_host) return fail(h, HYDRO_EINVAL, "null output");
+    DeviceGuard guard(h->device);
     for (int c = 0; c < K_NCLASS; ++c) { ms_host[c] = 0.0; count_host[c] = 0; }
     cudaError_t e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, HYDRO_ECUDA, std::string("profile_read: ") + cudaGetErrorString(e));
     for (auto &ev : h->events) {
         float ms = 0.f;
-        if (cudaEventElapsedTime(&ms, ev.a, ev.b) == cudaSuccess) { ms_host[ev.klass] += ms; count_host[ev.klass]++; }
-        cudaEventDestroy(ev.a); cudaEventDestroy(ev.b);
+        if (cudaEventElapsedTime(&ms, h->pool[ev.a], h->pool[ev.b]) == cudaSuccess) { ms_host[ev.klass] += ms; count_host[ev.klass]++; }
     }
     h->events.clear();
+    h->pool_used = 0;
     return HYDRO_OK;
 }
 
 int hydro_destroy(hydro_handle h)
 {
     if (!h) return HYDRO_OK;
+    DeviceGuard guard(h->device);
     cudaStreamSynchronize(h->stream);
-    for (auto &ev : h->events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    for (auto &ev : h->pool) cudaEventDestroy(ev);
     if (h->pinned) cudaFreeHost(h->pinned);
     delete h;
     return HYDRO_OK;
 }
 
 const char *hydro_last_error(hydro_handle h) { return h ? h->err.c_str() : g_init_error.c_str(); }
-
-int hydro_fp64_probe(double *rates_host)
-{
-    if (!rates_host) return fail(nullptr, HYDRO_EINVAL, "null rates_host");
-    const int blocks = 148 * 8, threads = 256, iters = 8192;
-    double *out = nullptr;
-    cudaEvent_t e0, e1;
-    if (cudaMalloc(&out, (size_t)blocks * threads * 8) != cudaSuccess)
-        return fail(nullptr, HYDRO_ENOMEM, "hydro_fp64_probe: device allocation failed");
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    int rc = HYDRO_OK;
-    for (int mode = 0; mode < 3 && rc == HYDRO_OK; ++mode) {
-        float best = 1e30f;
-        for (int rep = 0; rep < 4; ++rep) {           // first repetition warms up
-            cudaEventRecord(e0);
-            if (mode == 0) k_fp64_probe<0><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
-            else if (mode == 1) k_fp64_probe<1><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
-            else k_fp64_probe<2><<<blocks, threads>>>(out, iters, 1e-9, 0.999999);
-            cudaEventRecord(e1);
-            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = fail(nullptr, HYDRO_ECUDA, "hydro_fp64_probe: kernel failed"); break; }
-            float ms = 0.f;
-            cudaEventElapsedTime(&ms, e0, e1);
-            if (rep > 0 && ms < best) best = ms;
-        }
-        // FP64 thread-instructions per second (one DFMA = one instruction)
-        rates_host[mode] = (double)blocks * threads * 8.0 * iters / (best * 1e-3);
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(out);
-    return rc;
-}
-
-int hydro_tma_probe(int columns, int ncomp, double *gbs_host)
-{
-    if (!gbs_host || ncomp < 1 || ncomp > 6) return fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: ncomp must be 1..6");
-    const long long rows = 128LL * 128 * 64;                       // valid rows of one component of config 5
-    double *buf = nullptr, *out = nullptr;
-    if (cudaMalloc(&buf, (size_t)136 * rows * ncomp * 8) != cudaSuccess || cudaMalloc(&out, (size_t)rows * 8) != cudaSuccess) {
-        if (buf) cudaFree(buf);
-        return fail(nullptr, HYDRO_ENOMEM, "hydro_tma_probe: device allocation failed");
-    }
-    cudaMemset(buf, 0, (size_t)136 * rows * ncomp * 8);
-    int rc;
-    switch (columns) {
-        case 2: rc = tma_probe_run<2, 8>(ncomp, buf, rows, out, gbs_host); break;
-        case 4: rc = tma_probe_run<4, 6>(ncomp, buf, rows, out, gbs_host); break;
-        case 8: rc = tma_probe_run<8, 4>(ncomp, buf, rows, out, gbs_host); break;
-        default: rc = fail(nullptr, HYDRO_EINVAL, "hydro_tma_probe: columns must be 2, 4 or 8");
-    }
-    cudaFree(out); cudaFree(buf);
-    return rc;
-}
 
 int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt_host, double *totals_host)
 {
@@ -762,11 +895,7 @@ int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt
     e = cudaMemcpy(U0, U_host, sb, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { rc = fail(nullptr, HYDRO_ECUDA, std::string("H2D: ") + cudaGetErrorString(e)); goto done; }
     if ((rc = hydro_init(p, U0, U1, sc, scb, nullptr, &h))) goto done;
-    for (int s = 0; s < nsteps && rc == HYDRO_OK; ++s) {
-        double dt = 0.0;
-        if (dt_host) { rc = hydro_step(h, 1, &dt); dt_host[s] = dt; }
-        else rc = hydro_step(h, 1, nullptr);
-    }
+    rc = hydro_step(h, nsteps, dt_host);
     if (rc == HYDRO_OK && totals_host) rc = hydro_conserved_totals(h, 0, totals_host);
     if (rc != HYDRO_OK) { g_init_error = h->err; goto done; }
     e = cudaMemcpy(U_host, U0, sb, cudaMemcpyDeviceToHost);

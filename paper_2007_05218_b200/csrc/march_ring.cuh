@@ -201,8 +201,9 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
 
     const int tid = threadIdx.x;
-    const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
-    const int b = blockIdx.z;
+    const int tiles = gridDim.x / g.nboxes;      // grid.x = (CTAs per box) * boxes
+    const int b = blockIdx.x / tiles;
+    const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x - b * tiles);
     const int m0 = blockIdx.y * a.seglen;
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
@@ -391,8 +392,9 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
 
     const int tid = threadIdx.x;
-    const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x);
-    const int b = blockIdx.z;
+    const int tiles = gridDim.x / g.nboxes;      // grid.x = (CTAs per box) * boxes
+    const int b = blockIdx.x / tiles;
+    const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x - b * tiles);
     const int m0 = blockIdx.y * a.seglen;
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
@@ -519,48 +521,6 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         __syncthreads();
         if (tid == 0 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
     }
-}
-
-// ---- TMA probe (measurement only, hydro_tma_probe) ------------------------------------------
-// Streams an FP64 array of `rows` x 128 valid columns (row pitch 136, the config-5 state row) through a
-// D-deep ring with {C columns, 128 rows} boxes of NC components per step: thread t of a 128-thread CTA owns
-// ROW t and reads its C values of every component -- the transposing access a thread-per-row march along
-// the contiguous direction would use.  Every value is summed so that the loads are not dead.
-template <int C, int D>
-__global__ void __launch_bounds__(128)
-k_tma_probe(const __grid_constant__ CUtensorMap tm, int nc, int ncols, double* out)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    double* ring = reinterpret_cast<double*>(smem_raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * nc * 128 * C * 8);
-    const int tid = threadIdx.x, nsteps = ncols / C;
-    auto issue = [&](int it) {
-        uint64_t* bar = &full[it % D];
-        mbar_expect_tx(bar, (uint32_t)(nc * 128 * C * 8));
-        for (int c = 0; c < nc; ++c)
-            asm volatile(
-                "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-                ::"r"(smem_u32(ring + ((size_t)(it % D) * nc + c) * 128 * C)), "l"(&tm), "r"(smem_u32(bar)), "r"(it * C),
-                "r"((int)blockIdx.x * 128), "r"(c) : "memory");
-    };
-    if (tid == 0) {
-        for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
-        mbar_fence_init();
-    }
-    __syncthreads();
-    if (tid == 0)
-        for (int it = 0; it < D && it < nsteps; ++it) issue(it);
-    double acc = 0.0;
-    for (int it = 0; it < nsteps; ++it) {
-        mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
-        const double* slot = ring + (size_t)(it % D) * nc * 128 * C;
-        for (int c = 0; c < nc; ++c)
-#pragma unroll
-            for (int q = 0; q < C; ++q) acc += slot[(c * 128 + tid) * C + q];
-        __syncthreads();
-        if (tid == 0 && it + D < nsteps) issue(it + D);
-    }
-    out[(size_t)blockIdx.x * 128 + tid] = acc;
 }
 
 }  // namespace hydro

@@ -50,15 +50,17 @@ k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* 
 {
     const int lane = threadIdx.x & 31;
     const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
-    // grid (nchunk * ceil(nb_y / WARPS), nb_z, boxes): the chunks of a row are consecutive blocks, the
-    // warps of a block are WARPS consecutive rows; one 32-bit division per warp (a flat 64-bit warp
+    // grid (nchunk * ceil(nb_y / WARPS) * boxes, nb_z): the chunks of a row are consecutive blocks, the
+    // warps of a block are WARPS consecutive rows; two 32-bit divisions per warp (a flat 64-bit warp
     // index cost ~150 instructions of division per warp, 8 % of the kernel)
-    const int jb = blockIdx.x / nchunk;
-    const int chunk = blockIdx.x - jb * nchunk;
+    const int per_box = gridDim.x / g.nboxes;
+    const int b = blockIdx.x / per_box;
+    const int rb = blockIdx.x - b * per_box;
+    const int jb = rb / nchunk;
+    const int chunk = rb - jb * nchunk;
     const int j = jb * WARPS + (threadIdx.x >> 5);
     if (j >= g.nb[1]) return;                          // whole warp leaves together
     const int k = blockIdx.y;
-    const int b = blockIdx.z;
 
     const int i = chunk * XW_VALID + lane - 3;         // valid-zone index of this lane
     int ip = i + g.ng;                                 // padded index

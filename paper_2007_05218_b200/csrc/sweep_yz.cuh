@@ -43,11 +43,13 @@ template <int DIR>
 __device__ __forceinline__ bool pencil(const Geom& g, int seglen, int& i, int& t, int& b, int& m0, int& m1)
 {
     constexpr int T = (DIR == 1) ? 2 : 1;              // the other transverse dimension
-    const int pid = blockIdx.x * blockDim.x + threadIdx.x;
+    // grid.x = (CTAs per box) * boxes: the box index rides in blockIdx.x (no 65535 limit)
+    const int tiles = gridDim.x / g.nboxes;
+    b = blockIdx.x / tiles;
+    const int pid = (blockIdx.x - b * tiles) * blockDim.x + threadIdx.x;
     if (pid >= g.nb[0] * g.nb[T]) return false;
     i = pid % g.nb[0];
     t = pid / g.nb[0];
-    b = blockIdx.z;
     m0 = blockIdx.y * seglen;
     m1 = min(m0 + seglen, g.nb[DIR]);
     return true;

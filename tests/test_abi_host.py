@@ -30,6 +30,18 @@ def test_header_symbols_all_exported(lib):
         assert hasattr(lib, name), name
 
 
+def test_probe_library_is_separate(lib):
+    """The FP64-pipe probe of bench.py is a library of its own: hydro.h declares no probe, and
+    hydro_probe.h's one symbol is exported by libhydro_probe_b200.so, not by the product."""
+    hdr = open(os.path.join(ROOT, "include", "hydro_probe.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(hydro_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(B.PROBE_EXPORTS)
+    P = B.probe_lib()
+    for name in declared:
+        assert hasattr(P, name) and not hasattr(lib, name)
+
+
 def test_struct_layout_matches_header():
     # 3+3+1+1+3+3 int32 = 56 bytes, then 3+3+1+1+3+1+1 doubles = 104 bytes, then flatten + evolve_eint
     assert C.sizeof(B.HydroParams) == 56 + 104 + 8 and B.HydroParams.flatten.offset == 160
