@@ -156,23 +156,40 @@ class ClockSampler(threading.Thread):
                 "samples": len(sm)}
 
 
-def oracle_sample(steps, warmup):
-    """The oracle, as it stands, on a bounded sample of the config-5 recipe: the 256^3 instance of the
-    same index-based generator (13 species, periodic, CFL 0.4) in 64^3 boxes."""
+def host_info():
+    model = "unknown"
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count()}
+
+
+def oracle_sample(steps, warmup, n=256, threads=None):
+    """The oracle, as it stands, on a bounded sample of the config-5 recipe: the n^3 instance of the
+    same index-based generator (13 species, periodic, CFL 0.4) in 64^3 boxes, on `threads` host threads
+    (None = all the cores OpenMP sees; the loop over boxes is the only parallel loop)."""
     from oracle import oracle_binding as O
-    wl = W.config(5, ndom=(256, 256, 256), nbox=(64, 64, 64))
+    wl = W.config(5, ndom=(n, n, n), nbox=(64, 64, 64))
     U0 = W.initial_state(wl, threads=8)
     U1 = np.zeros_like(U0)
     p = O.make_params(wl.params)
+    all_threads = O.max_threads()
+    O.set_threads(threads or all_threads)
+    used = min(threads or all_threads, wl.nboxes)
     for _ in range(warmup):
         O.step(p, U0, U1)
     t0 = time.perf_counter()
     for _ in range(steps):
         O.step(p, U0, U1)
     el = time.perf_counter() - t0
-    return {"value": wl.zones * steps / el, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
-            "sample": f"config-5 recipe at 256^3 (13 species, 64 boxes of 64^3), {steps} RK2 steps, "
-                      f"OpenMP over boxes, {el:.1f} s"}, el / steps * 1e3, wl
+    O.set_threads(all_threads)
+    return {"value": wl.zones * steps / el, "unit": UNIT, "cores": used, "kind": "oracle",
+            "sample": f"config-5 recipe at {n}^3 (13 species, {wl.nboxes} boxes of 64^3), {steps} RK2 steps, "
+                      f"{used} thread(s) over boxes, {el:.1f} s"}, el / steps * 1e3, wl
 
 
 def workload_config(wl, n_cfg):
@@ -186,18 +203,30 @@ def workload_config(wl, n_cfg):
 
 # ----------------------------------------------------------------------------- reference arm
 def run_reference(args, rank):
+    """There is no reference implementation (paper text only): this arm times the CPU oracle, as it stands, on
+    this box's host cores.  `config` is the workload of our arm (the metric is a rate per zone); a STEP of this
+    arm is one RK2 step of a BOUNDED SAMPLE of it -- the 256^3 instance of the same index-based recipe (one eighth
+    of the zones, about 6 s on 16 cores; 128^3 when more than 24 steps are asked for) -- and `config.sample`,
+    `cpu_baseline.sample` and `ms_per_step` describe that sample, so that K + W steps end within a few minutes."""
     if rank != 0:
         return
-    steps = max(1, min(args.steps, 2))
-    cb, ms, wl = oracle_sample(steps, min(args.warmup, 1))
-    wl5 = W.config(args.config)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)
+    n = 256 if steps + warmup <= 24 else 128
+    cb, ms, wl = oracle_sample(steps, warmup, n=n)
+    cb.update(host_info())
+    cfg = workload_config(W.config(args.config), args.config)
+    cfg["l2_policy"] = "n/a (host)"
+    cfg["sample"] = {"workload": workload_config(wl, args.config)["workload"], "zones": wl.zones,
+                     "state_gb": round(wl.state_bytes / 1e9, 3),
+                     "why": "the oracle needs about 50 s per RK2 step of the 512^3 state on 16 cores; its rate per zone "
+                            "does not depend on the zone count"}
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True,
+            "steps": steps, "warmup": warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl5, args.config), "cpu_baseline": cb,
+            "config": cfg, "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "note": "no reference implementation exists (paper text only): this arm is the CPU oracle on a bounded "
-                    "sample of the workload"}
+            "note": "no reference implementation exists (paper text only): this arm is the CPU oracle; ms_per_step is the "
+                    "time of one step of config.sample, not of the 512^3 state"}
     print(json.dumps(line), flush=True)
 
 
@@ -288,49 +317,76 @@ def run_ours(args, rank, world, local_rank):
                                "gbs": step_alg / 1e9 / (ms_step * 1e-3),
                                "frac": step_alg / 1e9 / (ms_step * 1e-3) / peak,
                                "frac_of_nominal_8000": step_alg / 1e9 / (ms_step * 1e-3) / 8000.0}}
-    # ncu figures of the committed capture (profiles/traffic.json): DRAM bytes and instruction counts per
-    # launch.  With the live launch durations they give the second roofline: FP64 pipe and issue slots.
+    # ncu figures of the committed capture (profiles/traffic.json, written by paper_2007_05218_b200.ncu_summary):
+    # DRAM bytes and instruction counts per launch of every class.  They are used ONLY while the capture's source
+    # hash equals that of the CUDA sources this run was built from; with the live launch durations they give
+    # traffic_ratio (measured / algorithmic bytes) and the second roofline: FP64 pipe and issue slots.
+    from paper_2007_05218_b200 import ncu_summary
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     fp64 = B.hydro_probe_fp64()                               # measured FP64 instr/s of this GPU, now
-    sm_max_hz = (sampler.summary().get("sm_max_mhz") or 1965.0) * 1e6
-    if os.path.exists(tr):
+    clocks = sampler.summary()
+    sm_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6            # median SM clock sampled under load
+    capture = "none"
+    if os.path.exists(tr) and not (args.flatten or args.evolve):
         try:
             t = json.load(open(tr)).get(wl.name, {})
-            roofline["traffic"] = t.get("dram_bytes", {}).get(dom)
-            for k, v in kernels.items():
-                wi, fi = t.get("warp_instr", {}).get(k), t.get("fp64_warp_instr", {}).get(k)
-                if wi and fi:
+            if t.get("source_sha256") == ncu_summary.source_sha():
+                capture = "profiles/traffic.json (source hash matches)"
+                for k, v in kernels.items():
+                    c = t["classes"].get(k)
+                    if not c:
+                        continue
                     sec = v["ms_per_launch"] * 1e-3
-                    v["fp64_pipe_frac"] = fi * 32 / sec / fp64["dfma"]
-                    v["issue_slot_frac"] = wi / sec / (148 * 4 * sm_max_hz)
-        except Exception:
-            pass
-    roofline["alu"] = {"fp64_peak_instr_per_s": fp64["dfma"], "fp64_peak_source": "hydro_probe_fp64 (libhydro_probe_b200: independent DFMA chains), this run",
-                       "fp64_pipe_frac": kernels[dom].get("fp64_pipe_frac"), "issue_slot_frac": kernels[dom].get("issue_slot_frac"),
-                       "note": "instruction counts from the committed ncu capture (profiles/traffic.json), durations live"}
+                    v["traffic"] = c["dram_bytes"]
+                    v["traffic_ratio"] = c["dram_bytes"] / alg[k]
+                    v["fp64_pipe_frac"] = c["fp64_warp_instr"] * 32 / sec / fp64["dfma"]
+                    v["issue_slot_frac"] = c["warp_instr"] / sec / (148 * 4 * sm_hz)
+            else:
+                capture = "profiles/traffic.json is from other sources (hash differs): not used"
+        except Exception as e:                                  # a malformed file must not kill the bench line
+            capture = f"profiles/traffic.json unreadable ({type(e).__name__})"
+    roofline["traffic"] = kernels[dom].get("traffic")
+    roofline["traffic_ratio"] = kernels[dom].get("traffic_ratio")
+    roofline["ncu_capture"] = capture
+    roofline["alu"] = {"fp64_peak_instr_per_s": fp64["dfma"],
+                       "fp64_peak_source": "hydro_probe_fp64 (libhydro_probe_b200: independent DFMA chains), this run",
+                       "issue_peak_warp_instr_per_s": 148 * 4 * sm_hz,
+                       "issue_peak_source": "148 SMs x 4 schedulers x the median SM clock sampled during the run",
+                       "fp64_pipe_frac": kernels[dom].get("fp64_pipe_frac"), "issue_slot_frac": kernels[dom].get("issue_slot_frac")}
+    isf = kernels[dom].get("issue_slot_frac")
+    if isf is not None and isf > kernels[dom]["frac"]:
+        # the dominant class is bound by instruction issue / the FP64 pipe, not by HBM: say so (the HBM figures stay)
+        roofline["bound_note"] = (f"{dom} issues {isf:.2f} of the SM issue slots and keeps the FP64 pipe "
+                                  f"{kernels[dom].get('fp64_pipe_frac'):.2f} busy while moving {kernels[dom]['frac']:.2f} of the "
+                                  "HBM peak: ALU/issue-bound (DESIGN.md sec. 5)")
 
-    # ---- e2e: host buffers through hydro_run_host ---------------------------------------
+    # ---- e2e: the same K steps through the C-ABI call that takes HOST buffers ------------------
+    # hydro_run_host(params, U_host, K): allocate, H2D of the whole state, K steps, D2H of the whole state, free --
+    # all inside the timed region.  PCIe moves 2 x 24.5 GB per call, so the per-step cost is the call's divided by K.
     del h
     torch.cuda.empty_cache()
     e2e = None
     if not args.no_e2e:
         p = B.make_params(wl.params)
-        n_e2e = max(1, min(args.steps, 2))
-        B.hydro_run_host(p, host, 1)                            # warm-up (allocations, first touch)
+        B.hydro_run_host(p, host, 1)                            # warm-up (first touch of the pinned pages)
         barrier()
         t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            B.hydro_run_host(p, host, 1)
+        B.hydro_run_host(p, host, args.steps)
         torch.cuda.synchronize(dev)
         el = time.perf_counter() - t0
         el = reduce_max(el, world, dev)
-        e2e = {"value": job_value(wl.zones, n_e2e, el * 1e3, world), "unit": UNIT, "h2d_bytes_per_step": wl.state_bytes,
-               "d2h_bytes_per_step": wl.state_bytes, "steps": n_e2e, "pinned_host": pinned,
-               "api": "hydro_run_host(params, U_host, 1 step)"}
+        e2e = {"value": job_value(wl.zones, args.steps, el * 1e3, world), "unit": UNIT,
+               "h2d_bytes_per_step": wl.state_bytes / args.steps, "d2h_bytes_per_step": wl.state_bytes / args.steps,
+               "h2d_bytes_per_call": wl.state_bytes, "d2h_bytes_per_call": wl.state_bytes,
+               "steps": args.steps, "seconds_per_call": el, "pinned_host": pinned,
+               "api": f"hydro_run_host(params, U_host, {args.steps}) -- one call: cudaMalloc, H2D, {args.steps} steps, D2H, cudaFree"}
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu_baseline, _, _ = oracle_sample(3, 0)      # about 18 s of host work
+        cpu_baseline, _, _ = oracle_sample(3, 0)      # about 18 s of host work on all cores
+        one, _, _ = oracle_sample(1, 0, n=128, threads=1)   # about 8 s on one core
+        cpu_baseline["one_core"] = {"value": one["value"], "unit": UNIT, "sample": one["sample"]}
+        cpu_baseline.update(host_info())
 
     if rank == 0:
         cfg = workload_config(wl, args.config)
@@ -343,7 +399,7 @@ def run_ours(args, rank, world, local_rank):
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
                 "zone_stages_per_s": 2 * value, "roofline": roofline, "kernels": kernels,
                 "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": int(launches),
-                "clocks": sampler.summary(), "dt_last": dt_last, "total_mass": totals[0]}
+                "clocks": clocks, "dt_last": dt_last, "total_mass": totals[0]}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -50,13 +50,18 @@ extern "C" {
 #define HYDRO_BC_PERIODIC 0
 #define HYDRO_BC_OUTFLOW  1
 #define HYDRO_BC_REFLECT  2
+#define HYDRO_BC_EXTERNAL 3  /* the face is shared with another shard of the MultiFab (another handle, usually another
+                                GPU): hydro_fill_ghosts leaves the ghost zones across it alone, hydro_unpack_halo
+                                fills them (PAPER.md:85-99 the boxes of a level are distributed
+                                over ranks that exchange ghost zones) */
 
 typedef struct {
     int32_t ndom[3];            /* zones in the domain (x,y,z)                               */
     int32_t nbox[3];            /* zones per box; must divide ndom (regular tiling)          */
     int32_t ng;                 /* ghost zones per side, >= 3 (the scheme reads 3)           */
     int32_t nspec;              /* passive species, >= 0                                     */
-    int32_t bc_lo[3], bc_hi[3]; /* HYDRO_BC_*; periodic must be set on both sides of a dim   */
+    int32_t bc_lo[3], bc_hi[3]; /* HYDRO_BC_*; periodic must be set on both sides of a dim; ndom, prob_lo and prob_hi
+                                   of a shard (EXTERNAL faces) describe the shard's own sub-domain */
     double  prob_lo[3], prob_hi[3]; /* physical domain; dx = (prob_hi-prob_lo)/ndom          */
     double  gamma, cfl;
     double  grav[3];            /* constant acceleration; {0,0,0} disables the source        */
@@ -134,6 +139,20 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
  * returns HYDRO_ESTATE if ANY step's maximum was not a positive finite number (the state is then
  * unusable), with or without dt_host.  nsteps = 0 is a no-op; nsteps < 0 is HYDRO_EINVAL. */
 int hydro_step(hydro_handle h, int nsteps, double *dt_host);
+
+/* Halo exchange of a sharded MultiFab (driver: paper_2007_05218_b200/sharded.py).
+ * A halo of dimension dim (0 x, 1 y, 2 z) is the ng layers next to a face over the FULL padded extent of the
+ * other two dimensions, all NVAR components, of every box on that face:
+ *   hydro_halo_bytes = NVAR * ng * NTa * NTb * NBa * NBb * 8   (a, b = the other two dimensions).
+ * hydro_pack_halo copies the VALID layers next to face (dim, side; side 0 low, 1 high) of state `which` into
+ * buf_dev; hydro_unpack_halo copies a buffer packed by the neighbour shard from ITS opposite face into the GHOST
+ * layers beyond (dim, side).  Exchanging x, then y, then z after hydro_fill_ghosts fills edges and corners
+ * through the earlier dimensions' ghosts.  buf_dev: caller-owned DEVICE memory of hydro_halo_bytes, 8-byte
+ * aligned.  Asynchronous on the handle's stream.  A handle with an EXTERNAL face refuses hydro_step (no exchange
+ * is possible between its stages): HYDRO_EINVAL. */
+size_t hydro_halo_bytes(const hydro_params *p, int dim);
+int hydro_pack_halo(hydro_handle h, int which, int dim, int side, void *buf_dev);
+int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *buf_dev);
 
 /* Which internal paths this handle uses (for bench accounting; they change no result):
  * what = 0: TMA-ring marching kernels (1) or the plain-load fallback (0);

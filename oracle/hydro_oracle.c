@@ -625,3 +625,310 @@ int oracle_max_threads(void)
     return 1;
 #endif
 }
+
+/* Number of host threads of the loop over boxes from now on (n >= 1); no effect without OpenMP.  Results do
+ * not depend on it bit for bit; bench.py uses it to time the oracle on one core as well as on all. */
+void oracle_set_threads(int n)
+{
+#ifdef _OPENMP
+    extern void omp_set_num_threads(int);
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* =====================================================================================================
+ * O12 (readings C1..C9): the unsplit corner-transport-upwind (CTU)
+ * update -- PPM reconstruction, characteristic tracing of the parabolas over the domain of dependence of
+ * each wave, transverse flux corrections of the face states, ONE conservative flux evaluation per step.
+ * This is the integrator family the paper's throughput numbers were measured with; the
+ * paper prints none of it, so every formula below is a reading:
+ *
+ *  C1  one step, ghosts filled (ng >= 3):  U(n+1) = U(n) + dt * ( -dFx*dxinv - dFy*dyinv - dFz*dzinv + S ),
+ *      association as O6; then the rho*e re-synchronisation of O7.  dt is O8's (sum form, S9).
+ *  C2  per direction and primitive (rho, u, v, w, p, X_k): the monotonised parabola (aL, aR) of O3/O4, with
+ *      da = aR - aL, a6 = 6*(a - 0.5*(aL + aR)).  For a wave of speed lam, sig = fabs(lam)*dt*dxinv:
+ *        Ip(lam) = lam > 0 ? aR - 0.5*sig*(da - (1 - (2/3)*sig)*a6) : aR      (average over the part of the
+ *        Im(lam) = lam < 0 ? aL + 0.5*sig*(da + (1 - (2/3)*sig)*a6) : aL       zone the wave sweeps; CW84 1.12)
+ *      with the three speeds lam = un - c, un, un + c of the ZONE (c = sqrt(gamma*p/rho), zone averages).
+ *  C3  state on the HIGH face of a zone (left state of face i+1/2), reference state and characteristic
+ *      projection (Miller & Colella 2002 form):  ref = Ip(un + c) of (rho, un, p) if un + c > 0, else the zone
+ *      average;  with d*m = ref - Ip(un - c), d*0 = ref - Ip(un), d*p = ref - Ip(un + c):
+ *        am = 0.5*(dpm/(rho*c) - dum)*(rho/c),  ap = 0.5*(dpp/(rho*c) + dup)*(rho/c),  a0 = drho0 - dp0/(c*c)
+ *        am = un - c > 0 ? -am : 0;  ap = un + c > 0 ? -ap : 0;  a0 = un > 0 ? -a0 : 0   (waves that reach the face)
+ *        rho_f = rho_ref + ap + am + a0;  un_f = un_ref + (ap - am)*(c/rho);  p_f = p_ref + (ap + am)*(c*c)
+ *      LOW face (right state of face i-1/2): the same with Im, ref = Im(un - c) if un - c < 0 else the zone
+ *      average, and the waves kept are those with negative speed.
+ *  C4  transverse velocities and mass fractions ride on the un wave: HIGH face Ip(un) if un > 0 else the zone
+ *      average; LOW face Im(un) if un < 0 else the zone average.
+ *  C5  floors rho >= small_dens, p >= small_pres on every face state (as O5 does inside the solver).
+ *  C6  first fluxes F1_d = HLLC (O5) of the traced states on every face of direction d whose two zones lie in
+ *      -1 .. nb of every direction.
+ *  C7  transverse correction in the 6-solve form (the 2-D CTU of Colella 1990 applied pairwise; no
+ *      intermediate corner solves -- Castro's 12-solve corner coupling is the alternative this reading does not
+ *      take): the face state of zone z for direction d is turned into conserved variables
+ *      (rho, rho*u, rho*v, rho*w, rho*E = p*gm1inv + 0.5*rho*|u|^2, rho*X_k), every d' != d subtracts
+ *      0.5*dt*dxinv_d' * (F1_d'[high face of z] - F1_d'[low face of z]), d' in ascending order, and the result
+ *      goes back to primitives (rho floored, p = max(gm1*(rho*E - 0.5*|m|^2/rho), small_pres)).
+ *  C8  gravity: every face state's velocity gets + 0.5*dt*g after C7;  S_m = rho(n)*g,
+ *      S_E = (m(n) + 0.5*dt*rho(n)*g) . g  (time-centred momentum: exact for a uniform state at rest).
+ *  C9  final fluxes F_d = HLLC of the corrected states on the faces of the valid zones; update C1.
+ *
+ * Pins (tests/test_oracle_ctu.py): P16 free stream bitwise; P17 Sod against the exact solution; P18 a linear
+ * density profile advected exactly (fails on a wrong sig factor or wave gate); P19 diagonal advection order;
+ * P20 conservation 1e-13; P21 decomposition invariance bitwise, axis permutation; P22 gravity closed form.
+ * Parity unpinned: behaviour when the floors of C5 / C7 trigger.
+ * ===================================================================================================== */
+static const double TWO3 = 2.0 / 3.0;
+
+/* conserved (rho, mx, my, mz, rhoE, rhoX_k) <-> primitive (rho, u, v, w, p, X_k), NQ = NFLUX entries */
+static void ctu_prim_to_cons(const oracle_params *p, int nspec, const double *q, double *Uc)
+{
+    const double gm1inv = 1.0 / (p->gamma - 1.0);
+    Uc[0] = q[0];
+    Uc[1] = q[0] * q[1]; Uc[2] = q[0] * q[2]; Uc[3] = q[0] * q[3];
+    Uc[4] = q[4] * gm1inv + HALF * q[0] * (q[1] * q[1] + q[2] * q[2] + q[3] * q[3]);
+    for (int s = 0; s < nspec; ++s) Uc[5 + s] = q[0] * q[5 + s];
+}
+
+static void ctu_cons_to_prim(const oracle_params *p, int nspec, const double *Uc, double *q)
+{
+    double rho = dmax(Uc[0], p->small_dens);
+    double rinv = 1.0 / rho;
+    q[0] = rho;
+    q[1] = Uc[1] * rinv; q[2] = Uc[2] * rinv; q[3] = Uc[3] * rinv;
+    double K = HALF * (Uc[1] * Uc[1] + Uc[2] * Uc[2] + Uc[3] * Uc[3]) * rinv;
+    q[4] = dmax((p->gamma - 1.0) * (Uc[4] - K), p->small_pres);
+    for (int s = 0; s < nspec; ++s) q[5 + s] = Uc[5 + s] * rinv;
+}
+
+/* C2: parabola averages over the domain of dependence of a wave */
+static double ctu_Ip(double lam, double dtdx, double a, double aL, double aR)
+{
+    if (!(lam > 0.0)) return aR;
+    double sig = fabs(lam) * dtdx;
+    double da = aR - aL, a6 = 6.0 * (a - HALF * (aL + aR));
+    return aR - HALF * sig * (da - (1.0 - TWO3 * sig) * a6);
+}
+
+static double ctu_Im(double lam, double dtdx, double a, double aL, double aR)
+{
+    if (!(lam < 0.0)) return aL;
+    double sig = fabs(lam) * dtdx;
+    double da = aR - aL, a6 = 6.0 * (a - HALF * (aL + aR));
+    return aL + HALF * sig * (da + (1.0 - TWO3 * sig) * a6);
+}
+
+/* C3 + C4 + C5: traced states of ONE zone along direction d.  a, aL, aR: NQ zone averages and parabola edges.
+ * qm: state on the low face (right state of face i-1/2), qp: state on the high face (left state of i+1/2). */
+void oracle_ctu_trace(int d, double gamma, double small_dens, double small_pres, int nspec, double dtdx,
+                      const double *a, const double *aL, const double *aR, double *qm, double *qp)
+{
+    const int nq = 5 + nspec, in = 1 + d;
+    const double rho = a[0], un = a[in], pr = a[4];
+    const double c = sqrt(gamma * pr / rho);
+    const double lam[3] = { un - c, un, un + c };
+    const int hv[3] = { 0, in, 4 };       /* rho, normal velocity, pressure */
+    for (int side = 0; side < 2; ++side) {            /* 0: low face (Im), 1: high face (Ip) */
+        double I[3][3];                                /* [wave][rho, un, p] */
+        for (int w = 0; w < 3; ++w)
+            for (int v = 0; v < 3; ++v)
+                I[w][v] = side ? ctu_Ip(lam[w], dtdx, a[hv[v]], aL[hv[v]], aR[hv[v]])
+                               : ctu_Im(lam[w], dtdx, a[hv[v]], aL[hv[v]], aR[hv[v]]);
+        double ref[3];
+        const int wr = side ? 2 : 0;                   /* the fastest wave towards this face */
+        const int reaches = side ? (lam[2] > 0.0) : (lam[0] < 0.0);
+        for (int v = 0; v < 3; ++v) ref[v] = reaches ? I[wr][v] : a[hv[v]];
+        double dum = ref[1] - I[0][1], dpm = ref[2] - I[0][2];
+        double drho0 = ref[0] - I[1][0], dp0 = ref[2] - I[1][2];
+        double dup = ref[1] - I[2][1], dpp = ref[2] - I[2][2];
+        double am = HALF * (dpm / (rho * c) - dum) * (rho / c);
+        double ap = HALF * (dpp / (rho * c) + dup) * (rho / c);
+        double a0 = drho0 - dp0 / (c * c);
+        if (side) {
+            am = lam[0] > 0.0 ? -am : 0.0; ap = lam[2] > 0.0 ? -ap : 0.0; a0 = lam[1] > 0.0 ? -a0 : 0.0;
+        } else {
+            am = lam[0] < 0.0 ? -am : 0.0; ap = lam[2] < 0.0 ? -ap : 0.0; a0 = lam[1] < 0.0 ? -a0 : 0.0;
+        }
+        double *qf = side ? qp : qm;
+        qf[0] = dmax(ref[0] + ap + am + a0, small_dens);
+        qf[in] = ref[1] + (ap - am) * (c / rho);
+        qf[4] = dmax(ref[2] + (ap + am) * (c * c), small_pres);
+        for (int v = 1; v < nq; ++v) {                 /* C4: passively advected variables */
+            if (v == in || v == 4) continue;
+            if (side) qf[v] = lam[1] > 0.0 ? ctu_Ip(lam[1], dtdx, a[v], aL[v], aR[v]) : a[v];
+            else qf[v] = lam[1] < 0.0 ? ctu_Im(lam[1], dtdx, a[v], aL[v], aR[v]) : a[v];
+        }
+    }
+}
+
+/* one CTU step of one box: Us = U(n) with ghosts filled, Uout = U(n+1) on the valid zones */
+static void ctu_box(const oracle_params *p, const geom_t *g, double dt, const double *Us, double *Uout)
+{
+    const int ng = g->ng, nq = g->nq, nflux = g->nflux, nvar = g->nvar, nspec = p->nspec;
+    const size_t cs = g->comp_stride;
+    const long st[3] = { 1, g->nt[0], (long)g->nt[0] * g->nt[1] };    /* padded strides */
+    const int has_grav = !(p->grav[0] == 0.0 && p->grav[1] == 0.0 && p->grav[2] == 0.0);
+    /* O2 on every padded zone */
+    double *q = (double *)malloc(sizeof(double) * cs * nq);
+    double *Uc = (double *)malloc(sizeof(double) * nvar);
+    double *qz = (double *)malloc(sizeof(double) * nq);
+    for (size_t z = 0; z < cs; ++z) {
+        for (int c = 0; c < nvar; ++c) Uc[c] = Us[c * cs + z];
+        oracle_cons_to_prim(p->gamma, p->small_dens, p->small_pres, nspec, Uc, qz);
+        for (int c = 0; c < nq; ++c) q[c * cs + z] = qz[c];
+    }
+    /* C2-C5: traced face states of every zone -1 .. nb (all three directions), per direction */
+    double *qm[3], *qp[3], *F1[3], *F2[3];
+    for (int d = 0; d < 3; ++d) {
+        qm[d] = (double *)calloc(cs * nq, sizeof(double));
+        qp[d] = (double *)calloc(cs * nq, sizeof(double));
+        F1[d] = (double *)calloc(cs * nflux, sizeof(double));      /* flux on the LOW face of a zone */
+        F2[d] = (double *)calloc(cs * nflux, sizeof(double));
+    }
+    int nmax = 0;
+    for (int d = 0; d < 3; ++d) if (g->nt[d] > nmax) nmax = g->nt[d];
+    double *line = (double *)malloc(sizeof(double) * nmax * nq);
+    double *sl = (double *)malloc(sizeof(double) * nmax);
+    double *ed = (double *)malloc(sizeof(double) * nmax);
+    double *lL = (double *)malloc(sizeof(double) * nmax * nq);
+    double *lR = (double *)malloc(sizeof(double) * nmax * nq);
+    double *za = (double *)malloc(sizeof(double) * nq), *zL = (double *)malloc(sizeof(double) * nq);
+    double *zR = (double *)malloc(sizeof(double) * nq), *zm = (double *)malloc(sizeof(double) * nq);
+    double *zp = (double *)malloc(sizeof(double) * nq), *Ff = (double *)malloc(sizeof(double) * nflux);
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        const int n = g->nb[d] + 6;                                  /* line zones -3 .. nb+2 */
+        const double dtdx = dt * g->dxinv[d];
+        for (int t2 = -1; t2 <= g->nb[d2]; ++t2)
+        for (int t1 = -1; t1 <= g->nb[d1]; ++t1) {
+            int ijk[3];
+            ijk[d1] = t1 + ng; ijk[d2] = t2 + ng;
+            for (int c = 0; c < nq; ++c) {
+                for (int m = 0; m < n; ++m) {
+                    ijk[d] = m - 3 + ng;
+                    line[c * nmax + m] = q[c * cs + zidx(g, ijk[0], ijk[1], ijk[2])];
+                }
+                oracle_ppm_line(line + c * nmax, n, sl, ed, lL + c * nmax, lR + c * nmax);
+            }
+            for (int m = 2; m <= n - 3; ++m) {                       /* zones -1 .. nb */
+                for (int c = 0; c < nq; ++c) { za[c] = line[c * nmax + m]; zL[c] = lL[c * nmax + m]; zR[c] = lR[c * nmax + m]; }
+                oracle_ctu_trace(d, p->gamma, p->small_dens, p->small_pres, nspec, dtdx, za, zL, zR, zm, zp);
+                ijk[d] = m - 3 + ng;
+                size_t z = zidx(g, ijk[0], ijk[1], ijk[2]);
+                for (int c = 0; c < nq; ++c) { qm[d][c * cs + z] = zm[c]; qp[d][c * cs + z] = zp[c]; }
+            }
+        }
+    }
+    /* C6: first fluxes on the low face of zones 0 .. nb along d, -1 .. nb across */
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        for (int t2 = -1; t2 <= g->nb[d2]; ++t2)
+        for (int t1 = -1; t1 <= g->nb[d1]; ++t1)
+        for (int m = 0; m <= g->nb[d]; ++m) {
+            int ijk[3];
+            ijk[d] = m + ng; ijk[d1] = t1 + ng; ijk[d2] = t2 + ng;
+            size_t z = zidx(g, ijk[0], ijk[1], ijk[2]);
+            for (int c = 0; c < nq; ++c) { zL[c] = qp[d][c * cs + z - st[d]]; zR[c] = qm[d][c * cs + z]; }
+            oracle_hllc(d, p->gamma, p->small_dens, p->small_pres, nspec, zL, zR, Ff);
+            for (int c = 0; c < nflux; ++c) F1[d][c * cs + z] = Ff[c];
+        }
+    }
+    /* C7-C9: corrected states and final fluxes on the low face of zones 0 .. nb along d, valid across */
+    double *Ucf = (double *)malloc(sizeof(double) * nflux);
+    for (int d = 0; d < 3; ++d) {
+        const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+        for (int t2 = 0; t2 < g->nb[d2]; ++t2)
+        for (int t1 = 0; t1 < g->nb[d1]; ++t1)
+        for (int m = 0; m <= g->nb[d]; ++m) {
+            int ijk[3];
+            ijk[d] = m + ng; ijk[d1] = t1 + ng; ijk[d2] = t2 + ng;
+            size_t z = zidx(g, ijk[0], ijk[1], ijk[2]);
+            for (int side = 0; side < 2; ++side) {                   /* 0: left state (zone m-1), 1: right (zone m) */
+                const size_t zz = side ? z : z - st[d];
+                const double *src = side ? qm[d] : qp[d];
+                double *dst = side ? zR : zL;
+                for (int c = 0; c < nq; ++c) za[c] = src[c * cs + zz];
+                ctu_prim_to_cons(p, nspec, za, Ucf);
+                for (int dd = 0; dd < 3; ++dd) {                     /* ascending d' != d */
+                    if (dd == d) continue;
+                    for (int c = 0; c < nflux; ++c)
+                        Ucf[c] = Ucf[c] - HALF * dt * g->dxinv[dd] * (F1[dd][c * cs + zz + st[dd]] - F1[dd][c * cs + zz]);
+                }
+                ctu_cons_to_prim(p, nspec, Ucf, dst);
+                if (has_grav)
+                    for (int e = 0; e < 3; ++e) dst[1 + e] = dst[1 + e] + HALF * dt * p->grav[e];
+            }
+            oracle_hllc(d, p->gamma, p->small_dens, p->small_pres, nspec, zL, zR, Ff);
+            for (int c = 0; c < nflux; ++c) F2[d][c * cs + z] = Ff[c];
+        }
+    }
+    /* C1 + C8 + O7 */
+    const double floor_rhoe = p->small_pres * (1.0 / (p->gamma - 1.0));
+    double *L = (double *)malloc(sizeof(double) * nflux);
+    for (int k = 0; k < g->nb[2]; ++k)
+    for (int j = 0; j < g->nb[1]; ++j)
+    for (int i = 0; i < g->nb[0]; ++i) {
+        size_t z = zidx(g, i + ng, j + ng, k + ng);
+        for (int c = 0; c < nflux; ++c)
+            L[c] = -(F2[0][c * cs + z + st[0]] - F2[0][c * cs + z]) * g->dxinv[0]
+                   - (F2[1][c * cs + z + st[1]] - F2[1][c * cs + z]) * g->dxinv[1]
+                   - (F2[2][c * cs + z + st[2]] - F2[2][c * cs + z]) * g->dxinv[2];
+        if (has_grav) {
+            double rho = Us[0 * cs + z];
+            for (int e = 0; e < 3; ++e) {
+                L[1 + e] += rho * p->grav[e];
+                L[4] += (Us[(1 + e) * cs + z] + HALF * dt * rho * p->grav[e]) * p->grav[e];
+            }
+        }
+        for (int c = 0; c < nflux; ++c) {
+            int sc = c < 5 ? c : c + 1;
+            Uout[sc * cs + z] = Us[sc * cs + z] + dt * L[c];
+        }
+        double rho = Uout[0 * cs + z], mx = Uout[1 * cs + z], my = Uout[2 * cs + z], mz = Uout[3 * cs + z];
+        double re = Uout[4 * cs + z] - HALF * (mx * mx + my * my + mz * mz) / rho;
+        if (re < floor_rhoe) re = floor_rhoe;
+        Uout[5 * cs + z] = re;
+    }
+    free(L); free(Ucf);
+    free(Ff); free(zp); free(zm); free(zR); free(zL); free(za);
+    free(lR); free(lL); free(ed); free(sl); free(line);
+    for (int d = 0; d < 3; ++d) { free(F2[d]); free(F1[d]); free(qp[d]); free(qm[d]); }
+    free(qz); free(Uc); free(q);
+}
+
+/* U0 <- one CTU step of U0 with the given dt (ghosts are filled here); U1 is work space of the same size */
+int oracle_ctu_step_fixed_dt(const oracle_params *p, double *U0, double *U1, double dt)
+{
+    geom_t g;
+    if (make_geom(p, &g) || !U0 || !U1) return -1;
+    if (p->flatten || p->evolve_eint) return -1;       /* the options O10 / O11 belong to the method-of-lines path */
+    int rc = oracle_fill_ghosts(p, U0);
+    if (rc) return rc;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int b = 0; b < g.nboxes; ++b) {
+        size_t off = (size_t)b * g.box_stride;
+        ctu_box(p, &g, dt, U0 + off, U1 + off);
+    }
+    /* copy the new valid zones back (ghosts of U0 keep the old values and are refilled by the next step) */
+    for (int b = 0; b < g.nboxes; ++b)
+        for (int c = 0; c < g.nvar; ++c)
+            for (int k = 0; k < g.nb[2]; ++k)
+            for (int j = 0; j < g.nb[1]; ++j)
+            for (int i = 0; i < g.nb[0]; ++i) {
+                size_t z = (size_t)b * g.box_stride + c * g.comp_stride + zidx(&g, i + g.ng, j + g.ng, k + g.ng);
+                U0[z] = U1[z];
+            }
+    return 0;
+}
+
+int oracle_ctu_step(const oracle_params *p, double *U0, double *U1, double *dt_out)
+{
+    double dt;
+    int rc = oracle_estimate_dt(p, U0, &dt);
+    if (rc) return rc;
+    if ((rc = oracle_ctu_step_fixed_dt(p, U0, U1, dt))) return rc;
+    if (dt_out) *dt_out = dt;
+    return 0;
+}

@@ -62,7 +62,13 @@ def lib():
         L.oracle_flatten_line.argtypes = [dp, dp, C.c_int, C.c_double, dp]
         L.oracle_hllc.restype = None
         L.oracle_hllc.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp]
+        L.oracle_ctu_step.argtypes = [pp, dp, dp, dp]
+        L.oracle_ctu_step_fixed_dt.argtypes = [pp, dp, dp, C.c_double]
+        L.oracle_ctu_trace.restype = None
+        L.oracle_ctu_trace.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_double, dp, dp, dp, dp, dp]
         L.oracle_max_threads.restype = C.c_int
+        L.oracle_set_threads.restype = None
+        L.oracle_set_threads.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -150,3 +156,26 @@ def hllc(direction, gamma, qL, qR, small_dens=1e-12, small_pres=1e-14):
 
 def max_threads():
     return lib().oracle_max_threads()
+
+
+def set_threads(n: int):
+    lib().oracle_set_threads(int(n))
+
+
+def ctu_step(p, U0, U1):
+    """One CTU step (O12) of U0 in place; returns dt."""
+    dt = C.c_double(0.0)
+    _check(lib().oracle_ctu_step(C.byref(p), _ptr(U0), _ptr(U1), C.byref(dt)), "ctu_step")
+    return dt.value
+
+
+def ctu_step_fixed_dt(p, U0, U1, dt):
+    _check(lib().oracle_ctu_step_fixed_dt(C.byref(p), _ptr(U0), _ptr(U1), dt), "ctu_step_fixed_dt")
+
+
+def ctu_trace(d, gamma, small_dens, small_pres, dtdx, a, aL, aR):
+    """Traced face states (qm, qp) of one zone (readings C2-C5)."""
+    a, aL, aR = (np.ascontiguousarray(x, dtype=np.float64) for x in (a, aL, aR))
+    qm, qp = np.zeros_like(a), np.zeros_like(a)
+    lib().oracle_ctu_trace(d, gamma, small_dens, small_pres, a.size - 5, dtdx, _ptr(a), _ptr(aL), _ptr(aR), _ptr(qm), _ptr(qp))
+    return qm, qp

@@ -15,7 +15,8 @@ LIB_PATH = os.environ.get("HYDRO_LIB") or os.path.join(HERE, "libhydro_b200.so")
 HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3, -4
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
-           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host"]
+           "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host",
+           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo"]
 PROBE_LIB_PATH = os.path.join(HERE, "libhydro_probe_b200.so")
 PROBE_EXPORTS = ["hydro_probe_fp64"]
 
@@ -84,6 +85,10 @@ def lib():
     L.hydro_last_error.restype = C.c_char_p
     L.hydro_last_error.argtypes = [vp]
     L.hydro_run_host.argtypes = [pp, vp, C.c_int, dp, dp]
+    L.hydro_halo_bytes.restype = C.c_size_t
+    L.hydro_halo_bytes.argtypes = [pp, C.c_int]
+    L.hydro_pack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    L.hydro_unpack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
     _lib = L
     return L
 
@@ -94,6 +99,10 @@ def hydro_state_bytes(p: HydroParams) -> int:
 
 def hydro_scratch_bytes(p: HydroParams) -> int:
     return lib().hydro_scratch_bytes(C.byref(p))
+
+
+def hydro_halo_bytes(p: HydroParams, dim: int) -> int:
+    return lib().hydro_halo_bytes(C.byref(p), dim)
 
 
 _probe = None
@@ -191,6 +200,13 @@ class Hydro:
         if all_dts:
             return list(out)[:nsteps]
         return out[nsteps - 1] if (want_dt and nsteps > 0) else (0.0 if want_dt else None)
+
+    def hydro_pack_halo(self, which, dim, side, buf):
+        """buf: device tensor of hydro_halo_bytes(params, dim) bytes (sharded.py)."""
+        self._check(lib().hydro_pack_halo(self.h, which, dim, side, buf.data_ptr()))
+
+    def hydro_unpack_halo(self, which, dim, side, buf):
+        self._check(lib().hydro_unpack_halo(self.h, which, dim, side, buf.data_ptr()))
 
     def hydro_launch_count(self):
         return lib().hydro_launch_count(self.h)

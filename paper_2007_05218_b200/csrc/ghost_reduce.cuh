@@ -6,7 +6,8 @@ namespace hydro {
 
 // ---- O1 ----------------------------------------------------------------------------
 // Global index along dimension d -> the valid global index that supplies it; flip is set
-// when a reflecting wall was crossed.
+// when a reflecting wall was crossed.  Returns -1 when the zone lies across an EXTERNAL face
+// (bc 3: it belongs to another shard and is filled by hydro_unpack_halo, not here).
 __device__ __forceinline__ int map_global(const Geom& g, int d, int gi, bool& flip)
 {
     const int n = g.ndom[d];
@@ -15,6 +16,7 @@ __device__ __forceinline__ int map_global(const Geom& g, int d, int gi, bool& fl
     const int bc = gi < 0 ? g.bc_lo[d] : g.bc_hi[d];
     if (bc == 0) return ((gi % n) + n) % n;
     if (bc == 1) return gi < 0 ? 0 : n - 1;
+    if (bc == 3) return -1;
     flip = true;
     return gi < 0 ? -1 - gi : 2 * n - 1 - gi;
 }
@@ -31,6 +33,7 @@ k_fill_ghosts(const __grid_constant__ Geom g, double* __restrict__ U)
     const int bi = b % g.NB[0], bj = (b / g.NB[0]) % g.NB[1], bk = b / (g.NB[0] * g.NB[1]);
     bool fz;
     const int gz = map_global(g, 2, bk * g.nb[2] + kl - g.ng, fz);
+    if (gz < 0) return;                                                // plane across an external z face
     const int sbk = gz / g.nb[2];
     const int skl = gz - sbk * g.nb[2] + g.ng;
     const bool kghost = kl < g.ng || kl >= g.ng + g.nb[2];
@@ -54,6 +57,7 @@ k_fill_ghosts(const __grid_constant__ Geom g, double* __restrict__ U)
         bool fx, fy;
         const int gx = map_global(g, 0, bi * g.nb[0] + il - g.ng, fx);
         const int gy = map_global(g, 1, bj * g.nb[1] + jl - g.ng, fy);
+        if (gx < 0 || gy < 0) continue;                                // across an external x or y face
         const int sbi = gx / g.nb[0], sbj = gy / g.nb[1];
         const long long sb = ((long long)sbk * g.NB[1] + sbj) * g.NB[0] + sbi;
         double v = splane[sb * g.bstride + (long long)(gy - sbj * g.nb[1] + g.ng) * g.nt[0] + (gx - sbi * g.nb[0] + g.ng)];
@@ -321,6 +325,39 @@ k_totals_final(const __grid_constant__ Geom g, const double* __restrict__ part, 
         dd_add(hi, lo, oh, ol);
     }
     if (threadIdx.x == 0) out[c] = (hi + lo) * g.vol;
+}
+
+// ---- halo layers of a sharded MultiFab (paper_2007_05218_b200/sharded.py) ------------------
+// A halo of dimension `dim` = the ng layers next to a face, over the FULL padded extent of the other two
+// dimensions, of every component of every box on that face: buffer layout [face box][component][t1][t0][layer]
+// for dim = 0 and [face box][component][layer][t1][t0] for dim = 1 (t0 = i, t1 = k) and dim = 2 (t0 = i, t1 = j);
+// face boxes ordered by their other two box coordinates, lower dimension fastest.  PACK reads the VALID layers
+// next to the face, UNPACK writes the GHOST layers beyond it.  One thread per double, grid-stride.
+template <bool PACK>
+__global__ void __launch_bounds__(256)
+k_halo(const __grid_constant__ Geom g, double* __restrict__ U, double* __restrict__ buf, int dim, int side)
+{
+    const int d0 = dim == 0 ? 1 : 0, d1 = dim == 2 ? 1 : 2;          // the other two dimensions, lower first
+    const long long n0 = g.nt[d0], n1 = g.nt[d1], ng = g.ng;
+    const long long per_comp = ng * n0 * n1, per_box = per_comp * g.nvar;
+    const long long total = per_box * g.NB[d0] * g.NB[d1];
+    const int lay0 = PACK ? (side == 0 ? g.ng : g.nb[dim]) : (side == 0 ? 0 : g.nb[dim] + g.ng);
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+        const long long fb = e / per_box;
+        long long r = e - fb * per_box;
+        const int c = (int)(r / per_comp);
+        r -= c * per_comp;
+        int l, t0, t1;
+        if (dim == 0) { l = (int)(r % ng); r /= ng; t0 = (int)(r % n0); t1 = (int)(r / n0); }
+        else { t0 = (int)(r % n0); r /= n0; t1 = (int)(r % n1); l = (int)(r / n1); }
+        int bc[3], pc[3];
+        bc[dim] = side == 0 ? 0 : g.NB[dim] - 1;
+        bc[d0] = (int)(fb % g.NB[d0]); bc[d1] = (int)(fb / g.NB[d0]);
+        pc[dim] = lay0 + l; pc[d0] = t0; pc[d1] = t1;
+        const long long b = ((long long)bc[2] * g.NB[1] + bc[1]) * g.NB[0] + bc[0];
+        const long long z = (b * g.nvar + c) * g.cstride + ((long long)pc[2] * g.nt[1] + pc[1]) * g.nt[0] + pc[0];
+        if (PACK) buf[e] = U[z]; else U[z] = buf[e];
+    }
 }
 
 }  // namespace hydro

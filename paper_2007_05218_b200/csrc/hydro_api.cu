@@ -95,6 +95,7 @@ struct hydro_ctx {
     bool fuse_dt;             // hydro_step: the stage-1 z hydro sweep also reduces the next step's dt
     CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
     CUtensorMap fmaps[2];      // [DIR-1]: TMA views of the flattening-coefficient array (flatten == 1)
+    bool external;             // some face is HYDRO_BC_EXTERNAL (sharded MultiFab)
     bool use_xmarch;           // x sweep by the marching kernels of march_x.cuh (else k_sweep_x)
     CUtensorMap xmaps[2][6];   // [state][components per box]: {4 zones, 128 rows} views for the x hydro marching kernel
     CUtensorMap xsmaps[2][6];  // the same with XS_ROWS rows per box, for the x species marching kernels
@@ -130,8 +131,8 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
         if (p->ndom[d] <= 0 || p->nbox[d] <= 0 || p->ndom[d] % p->nbox[d] != 0) {
             why = "nbox must be positive and divide ndom"; return false;
         }
-        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 2 || p->bc_hi[d] < 0 || p->bc_hi[d] > 2) {
-            why = "bc must be 0, 1 or 2"; return false;
+        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 3 || p->bc_hi[d] < 0 || p->bc_hi[d] > 3) {
+            why = "bc must be 0, 1, 2 or 3"; return false;
         }
         if ((p->bc_lo[d] == HYDRO_BC_PERIODIC) != (p->bc_hi[d] == HYDRO_BC_PERIODIC)) {
             why = "periodic must be set on both sides of a dimension"; return false;
@@ -735,10 +736,14 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
         return fail(nullptr, HYDRO_EINVAL, "evolve_eint = 1 needs a geometry the TMA-ring kernels accept "
                                            "(even ng, even nbox[0] that divides or is a multiple of 128)");
     }
+    // a face shared with another shard (HYDRO_BC_EXTERNAL): its ghosts come from hydro_unpack_halo; only the
+    // one-launch ghost fill knows how to leave them alone, and hydro_step (no exchange between its stages) is refused
+    h->external = false;
+    for (int d = 0; d < 3; ++d) h->external = h->external || p->bc_lo[d] == HYDRO_BC_EXTERNAL || p->bc_hi[d] == HYDRO_BC_EXTERNAL;
     // split ghost fill inside hydro_step: needs the ring kernels, 16-byte rows and boxes >= ng wide
     h->fuse_dt = h->use_ring && !g.evolve && h->kn.fuse_dt != 0;   // O11: rho*e is final only after the energy kernel
     h->split_ghosts = h->use_ring && (g.nt[0] % 2 == 0) && g.nb[0] >= g.ng && g.nb[1] >= g.ng && g.nb[2] >= g.ng &&
-                      h->kn.split_ghosts != 0;
+                      h->kn.split_ghosts != 0 && !h->external;
     const size_t npin = (size_t)(g.nflux > 2 * DT_SLOTS ? g.nflux : 2 * DT_SLOTS);
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->pinned, npin * 8);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->scratch + cv.red, 0, 256, h->stream);
@@ -808,6 +813,9 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_host)
 {
     if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
     if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
+    if (h->external)
+        return fail(h, HYDRO_EINVAL, "hydro_step cannot run on a shard (HYDRO_BC_EXTERNAL faces need a halo exchange "
+                                     "between the stages): call the stages one by one");
     DeviceGuard guard(h->device);
     for (int done = 0; done < nsteps; done += DT_SLOTS) {
         const int n = nsteps - done < DT_SLOTS ? nsteps - done : DT_SLOTS;
@@ -815,6 +823,35 @@ int hydro_step(hydro_handle h, int nsteps, double *dt_host)
         if (rc) return rc;
     }
     return HYDRO_OK;
+}
+
+size_t hydro_halo_bytes(const hydro_params *p, int dim)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why) || dim < 0 || dim > 2) return 0;
+    const int d0 = dim == 0 ? 1 : 0, d1 = dim == 2 ? 1 : 2;
+    return (size_t)g.nvar * g.ng * g.nt[d0] * g.nt[d1] * g.NB[d0] * g.NB[d1] * 8;
+}
+
+static int halo_impl(hydro_handle h, int which, int dim, int side, void *buf_dev, bool pack)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if ((which != 0 && which != 1) || dim < 0 || dim > 2 || (side != 0 && side != 1))
+        return fail(h, HYDRO_EINVAL, "which and side must be 0 or 1, dim 0..2");
+    if (!buf_dev || ((uintptr_t)buf_dev & 7)) return fail(h, HYDRO_EINVAL, "null or misaligned halo buffer");
+    if (h->g.nb[dim] < h->g.ng) return fail(h, HYDRO_EINVAL, "boxes narrower than ng cannot supply a halo");
+    DeviceGuard guard(h->device);
+    prof_begin(h);
+    if (pack) k_halo<true><<<RED_BLOCKS, 256, 0, h->stream>>>(h->g, h->U[which], (double *)buf_dev, dim, side);
+    else k_halo<false><<<RED_BLOCKS, 256, 0, h->stream>>>(h->g, h->U[which], (double *)buf_dev, dim, side);
+    return check_launch(h, pack ? "k_halo<pack>" : "k_halo<unpack>", K_GHOST);
+}
+
+int hydro_pack_halo(hydro_handle h, int which, int dim, int side, void *buf_dev) { return halo_impl(h, which, dim, side, buf_dev, true); }
+
+int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *buf_dev)
+{
+    return halo_impl(h, which, dim, side, const_cast<void *>(buf_dev), false);
 }
 
 int hydro_query(hydro_handle h, int what)
