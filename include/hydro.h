@@ -140,6 +140,17 @@ int hydro_conserved_totals(hydro_handle h, int which, double *totals_host);
  * unusable), with or without dt_host.  nsteps = 0 is a no-op; nsteps < 0 is HYDRO_EINVAL. */
 int hydro_step(hydro_handle h, int nsteps, double *dt_host);
 
+/* O12 (the integrator family behind PAPER.md:79 and :89): n steps of
+ * the unsplit corner-transport-upwind update -- PPM, characteristic tracing, transverse flux corrections, ONE
+ * conservative flux evaluation per step -- each step = { estimate_dt; fill ghosts; CTU update }, dt kept on the
+ * device.  U0 is advanced in place (U1 is work space); dt_host and the HYDRO_ESTATE rule as for hydro_step.
+ * ctu_scratch_dev: caller-owned DEVICE memory, 16-byte aligned, of at least hydro_ctu_scratch_bytes (the traced
+ * states and fluxes of ONE box: 12 * NFLUX padded arrays); the boxes are worked through in batches of as many
+ * boxes as the buffer holds, so a larger buffer means fewer, larger launches.  Not available with the options
+ * flatten / evolve_eint or on a shard (HYDRO_EINVAL). */
+size_t hydro_ctu_scratch_bytes(const hydro_params *p);
+int hydro_ctu_step(hydro_handle h, void *ctu_scratch_dev, size_t ctu_scratch_bytes, int nsteps, double *dt_host);
+
 /* Halo exchange of a sharded MultiFab (driver: paper_2007_05218_b200/sharded.py).
  * A halo of dimension dim (0 x, 1 y, 2 z) is the ng layers next to a face over the FULL padded extent of the
  * other two dimensions, all NVAR components, of every box on that face:
@@ -175,8 +186,8 @@ long long hydro_launch_count(hydro_handle h);
  * hydro_profile_read synchronises, then writes the summed device time in ms and the launch
  * count of each kernel class into ms_host[HYDRO_NCLASS] / count_host[HYDRO_NCLASS] and clears the record.
  * Classes: 0 ghost fill, 1 dt reduction, 2 x sweep, 3 y hydro sweep, 4 y species sweep,
- * 5 z hydro sweep + update, 6 z species sweep + update, 7 totals, 8 flattening coefficients. */
-#define HYDRO_NCLASS 9
+ * 5 z hydro sweep + update, 6 z species sweep + update, 7 totals, 8 flattening coefficients, 9 CTU kernels. */
+#define HYDRO_NCLASS 10
 int hydro_profile(hydro_handle h, int enable);
 int hydro_profile_read(hydro_handle h, double *ms_host, long long *count_host);
 

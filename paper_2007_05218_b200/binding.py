@@ -16,7 +16,7 @@ HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3,
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
            "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host",
-           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo"]
+           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo", "hydro_ctu_scratch_bytes", "hydro_ctu_step"]
 PROBE_LIB_PATH = os.path.join(HERE, "libhydro_probe_b200.so")
 PROBE_EXPORTS = ["hydro_probe_fp64"]
 
@@ -85,6 +85,9 @@ def lib():
     L.hydro_last_error.restype = C.c_char_p
     L.hydro_last_error.argtypes = [vp]
     L.hydro_run_host.argtypes = [pp, vp, C.c_int, dp, dp]
+    L.hydro_ctu_scratch_bytes.restype = C.c_size_t
+    L.hydro_ctu_scratch_bytes.argtypes = [pp]
+    L.hydro_ctu_step.argtypes = [vp, vp, C.c_size_t, C.c_int, dp]
     L.hydro_halo_bytes.restype = C.c_size_t
     L.hydro_halo_bytes.argtypes = [pp, C.c_int]
     L.hydro_pack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
@@ -99,6 +102,10 @@ def hydro_state_bytes(p: HydroParams) -> int:
 
 def hydro_scratch_bytes(p: HydroParams) -> int:
     return lib().hydro_scratch_bytes(C.byref(p))
+
+
+def hydro_ctu_scratch_bytes(p: HydroParams) -> int:
+    return lib().hydro_ctu_scratch_bytes(C.byref(p))
 
 
 def hydro_halo_bytes(p: HydroParams, dim: int) -> int:
@@ -201,6 +208,20 @@ class Hydro:
             return list(out)[:nsteps]
         return out[nsteps - 1] if (want_dt and nsteps > 0) else (0.0 if want_dt else None)
 
+    def hydro_ctu_step(self, nsteps=1, batch_boxes=None, all_dts=False):
+        """nsteps CTU steps (O12).  The scratch for `batch_boxes` boxes (default: as many as fit in 40 GB, at least
+        one) is allocated on first use and kept."""
+        per_box = lib().hydro_ctu_scratch_bytes(C.byref(self.p))
+        nboxes = 1
+        for d in range(3):
+            nboxes *= self.p.ndom[d] // self.p.nbox[d]
+        nb = batch_boxes or max(1, min(nboxes, int(40e9 // per_box)))
+        if getattr(self, "_ctu", None) is None or self._ctu.numel() < nb * per_box:
+            self._ctu = self.torch.empty(nb * per_box, dtype=self.torch.uint8, device=self.device)
+        out = (C.c_double * max(nsteps, 1))()
+        self._check(lib().hydro_ctu_step(self.h, self._ctu.data_ptr(), nb * per_box, nsteps, out))
+        return list(out)[:nsteps] if all_dts else (out[nsteps - 1] if nsteps > 0 else 0.0)
+
     def hydro_pack_halo(self, which, dim, side, buf):
         """buf: device tensor of hydro_halo_bytes(params, dim) bytes (sharded.py)."""
         self._check(lib().hydro_pack_halo(self.h, which, dim, side, buf.data_ptr()))
@@ -215,14 +236,14 @@ class Hydro:
         return lib().hydro_query(self.h, what)
 
     KERNEL_CLASSES = ["fill_ghosts", "estimate_dt", "sweep_x", "hydro_y", "species_y", "hydro_z", "species_z",
-                      "totals", "flatten"]
+                      "totals", "flatten", "ctu"]
 
     def hydro_profile(self, enable):
         self._check(lib().hydro_profile(self.h, int(enable)))
 
     def hydro_profile_read(self):
-        ms = (C.c_double * 9)()
-        cnt = (C.c_longlong * 9)()
+        ms = (C.c_double * 10)()
+        cnt = (C.c_longlong * 10)()
         self._check(lib().hydro_profile_read(self.h, ms, cnt))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.KERNEL_CLASSES)}
 

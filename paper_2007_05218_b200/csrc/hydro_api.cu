@@ -18,6 +18,7 @@
 #include "sweep_yz.cuh"
 #include "march_ring.cuh"
 #include "march_x.cuh"
+#include "ctu.cuh"
 
 using namespace hydro;
 
@@ -258,7 +259,7 @@ int fail(hydro_handle h, int code, const std::string &msg)
 }
 
 // kernel classes of hydro_profile_read
-enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIES_Z, K_TOTALS, K_FLATTEN, K_NCLASS };
+enum { K_GHOST = 0, K_DT, K_SWEEP_X, K_HYDRO_Y, K_SPECIES_Y, K_HYDRO_Z, K_SPECIES_Z, K_TOTALS, K_FLATTEN, K_CTU, K_NCLASS };
 
 void prof_begin(hydro_handle h)
 {
@@ -583,13 +584,13 @@ int fill_ghost_rows_impl(hydro_handle h, int which)
 // validates every step's max t after the chunk
 double *dt_slot(hydro_handle h, int slot) { return (double *)(h->scratch + h->cv.dtslot) + 2 * (slot % DT_SLOTS); }
 
-int launch_dt(hydro_handle h, int slot = 0)
+int launch_dt(hydro_handle h, int slot = 0, int which = 0)
 {
     const long long nrows = (long long)h->g.nb[1] * h->g.nb[2] * h->g.nboxes;
     long long blocks = (nrows + 7) / 8;            // 8 warps per block, one row per warp and trip
     if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
     prof_begin(h);
-    k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[0],
+    k_estimate_dt<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->U[which],
                                                            (unsigned long long *)(h->scratch + h->cv.red),
                                                            dt_slot(h, slot));
     return check_launch(h, "k_estimate_dt", K_DT);
@@ -628,6 +629,68 @@ int step_chunk(hydro_handle h, int nsteps, double *dt_host)
         if ((rc = split ? fill_ghost_rows_impl(h, 1) : fill_ghosts_impl(h, 1))) return rc;
         double *dt_next = (fuse && s + 1 < nsteps) ? dt_slot(h, s + 1) : nullptr;
         if ((rc = advance_stage_impl(h, 1, 0.0, dt_dev, split, dt_next))) return rc;
+    }
+    return read_dts(h, dt_host, nsteps);
+}
+
+// ---- O12: CTU step (ctu.cuh) --------------------------------------------------------------------------------
+size_t ctu_box_bytes(const Geom &g) { return (size_t)12 * g.nflux * g.cstride * 8; }
+
+template <int DIR>
+int ctu_dir(hydro_handle h, const CtuArgs &a, int phase)
+{
+    const Geom &g = h->g;
+    const int nb[3] = {g.nb[0], g.nb[1], g.nb[2]};
+    auto grid = [&](int ext, int face, int ncomp) {
+        int n[3] = {nb[0] + 2 * ext, nb[1] + 2 * ext, nb[2] + 2 * ext};
+        if (face >= 0) n[face] = nb[face] + 1;
+        return dim3((unsigned)(((n[0] + 31) / 32) * a.nbatch), (unsigned)(n[1] * ncomp), (unsigned)n[2]);
+    };
+    int rc = HYDRO_OK;
+    const int ns = g.nspec;
+    prof_begin(h);
+    if (phase == 0) k_ctu_trace_hydro<DIR><<<grid(1, -1, 1), 32, 0, h->stream>>>(g, a);
+    else if (phase == 1) k_ctu_flux_hydro<DIR, false><<<grid(1, DIR, 1), 32, 0, h->stream>>>(g, a);
+    else k_ctu_flux_hydro<DIR, true><<<grid(0, DIR, 1), 32, 0, h->stream>>>(g, a);
+    if ((rc = check_launch(h, "k_ctu hydro", K_CTU))) return rc;
+    if (ns > 0) {
+        prof_begin(h);
+        if (phase == 0) k_ctu_trace_species<DIR><<<grid(1, -1, ns), 32, 0, h->stream>>>(g, a);
+        else if (phase == 1) k_ctu_flux_species<DIR, false><<<grid(1, DIR, ns), 32, 0, h->stream>>>(g, a);
+        else k_ctu_flux_species<DIR, true><<<grid(0, DIR, ns), 32, 0, h->stream>>>(g, a);
+        rc = check_launch(h, "k_ctu species", K_CTU);
+    }
+    return rc;
+}
+
+int ctu_chunk(hydro_handle h, char *scratch, size_t bytes, int nsteps, double *dt_host, int &cur)
+{
+    const Geom &g = h->g;
+    int nbatch_max = (int)(bytes / ctu_box_bytes(g));
+    if (nbatch_max > g.nboxes) nbatch_max = g.nboxes;
+    int rc;
+    for (int s = 0; s < nsteps; ++s) {
+        if ((rc = launch_dt(h, s, cur))) return rc;
+        if ((rc = fill_ghosts_impl(h, cur))) return rc;
+        for (int box0 = 0; box0 < g.nboxes; box0 += nbatch_max) {
+            CtuArgs a;
+            a.U = h->U[cur]; a.Unew = h->U[cur ^ 1]; a.Q = (double *)scratch; a.dt_dev = dt_slot(h, s);
+            a.box0 = box0; a.nbatch = g.nboxes - box0 < nbatch_max ? g.nboxes - box0 : nbatch_max;
+            for (int phase = 0; phase < 3; ++phase) {
+                if ((rc = ctu_dir<0>(h, a, phase))) return rc;
+                if ((rc = ctu_dir<1>(h, a, phase))) return rc;
+                if ((rc = ctu_dir<2>(h, a, phase))) return rc;
+            }
+            prof_begin(h);
+            k_ctu_update_hydro<<<dim3((unsigned)(((g.nb[0] + 31) / 32) * a.nbatch), g.nb[1], g.nb[2]), 32, 0, h->stream>>>(g, a);
+            if ((rc = check_launch(h, "k_ctu_update_hydro", K_CTU))) return rc;
+            if (g.nspec > 0) {
+                prof_begin(h);
+                k_ctu_update_species<<<dim3((unsigned)(((g.nb[0] + 31) / 32) * a.nbatch), g.nb[1] * g.nspec, g.nb[2]), 32, 0, h->stream>>>(g, a);
+                if ((rc = check_launch(h, "k_ctu_update_species", K_CTU))) return rc;
+            }
+        }
+        cur ^= 1;
     }
     return read_dts(h, dt_host, nsteps);
 }
@@ -852,6 +915,38 @@ int hydro_pack_halo(hydro_handle h, int which, int dim, int side, void *buf_dev)
 int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *buf_dev)
 {
     return halo_impl(h, which, dim, side, const_cast<void *>(buf_dev), false);
+}
+
+size_t hydro_ctu_scratch_bytes(const hydro_params *p)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why)) return 0;
+    return ctu_box_bytes(g);
+}
+
+int hydro_ctu_step(hydro_handle h, void *ctu_scratch_dev, size_t ctu_scratch_bytes, int nsteps, double *dt_host)
+{
+    if (!h) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    if (nsteps < 0) return fail(h, HYDRO_EINVAL, "nsteps must be >= 0");
+    const Geom &g = h->g;
+    if (g.flatten || g.evolve) return fail(h, HYDRO_EINVAL, "the options flatten / evolve_eint belong to the method-of-lines path");
+    if (h->external) return fail(h, HYDRO_EINVAL, "hydro_ctu_step cannot run on a shard (HYDRO_BC_EXTERNAL)");
+    if (!ctu_scratch_dev || ((uintptr_t)ctu_scratch_dev & 15)) return fail(h, HYDRO_EINVAL, "null or misaligned CTU scratch");
+    if (ctu_scratch_bytes < ctu_box_bytes(g)) return fail(h, HYDRO_ENOMEM, "ctu_scratch_bytes too small (hydro_ctu_scratch_bytes)");
+    if ((long long)(g.nb[1] + 2) * (g.nspec > 0 ? g.nspec : 1) > 65535 || g.nb[2] + 2 > 65535)
+        return fail(h, HYDRO_EINVAL, "CTU grid too large (nbox[1] * nspec or nbox[2])");
+    DeviceGuard guard(h->device);
+    int cur = 0, rc = HYDRO_OK;
+    for (int done = 0; done < nsteps && rc == HYDRO_OK; done += DT_SLOTS) {
+        const int n = nsteps - done < DT_SLOTS ? nsteps - done : DT_SLOTS;
+        rc = ctu_chunk(h, (char *)ctu_scratch_dev, ctu_scratch_bytes, n, dt_host ? dt_host + done : nullptr, cur);
+    }
+    if (cur == 1) {     // an odd number of steps left the result in U1: the contract is "U0 advanced in place"
+        cudaError_t e = cudaMemcpyAsync(h->U[0], h->U[1], (size_t)g.bstride * g.nboxes * 8, cudaMemcpyDeviceToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess && rc == HYDRO_OK) rc = fail(h, HYDRO_ECUDA, std::string("CTU copy back: ") + cudaGetErrorString(e));
+    }
+    return rc;
 }
 
 int hydro_query(hydro_handle h, int what)

@@ -55,4 +55,19 @@ for name, make in CASES[:3]:
     print(name, "xmarch", "bitwise" if ok else "DIFFERS", flush=True)
     if not ok:
         bad.append((name, "xmarch"))
+# the CTU update O12: strict build == oracle_ctu_step, bit for bit
+os.environ["HYDRO_XMARCH"] = "0"
+for name, make in CASES:
+    wl = make()
+    h = Hydro(wl.params)
+    U0 = W.initial_state(wl)
+    h.upload(U0, 0)
+    p = O.make_params(wl.params)
+    Uo, T = U0.copy(), np.zeros_like(U0)
+    dts_o = [O.ctu_step(p, Uo, T) for _ in range(3)]
+    dts_g = h.hydro_ctu_step(3, all_dts=True)
+    ok = dts_o == dts_g and np.array_equal(W.gather_valid(wl, h.download(0).reshape(U0.shape)), W.gather_valid(wl, Uo))
+    print(name, "ctu", "bitwise" if ok else "DIFFERS", flush=True)
+    if not ok:
+        bad.append((name, "ctu"))
 sys.exit(1 if bad else 0)
