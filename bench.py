@@ -230,6 +230,51 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def run_ctu(args, wl, h, host, t_gen, barrier, local_rank, world, dev):
+    """--ctu: the CTU update O12.  A step = one hydro_ctu_step step: estimate_dt, ghost fill,
+    ONE flux evaluation (6 Riemann solves per zone) and update.  First CUDA path of the row: its kernels keep the traced
+    states and fluxes in HBM, so the roofline object is the whole step's measured-by-model bytes, not a tuned kernel's."""
+    import torch
+    per_box = 12 * wl.nflux * int(np.prod(wl.nt)) * 8
+    nb = max(1, min(wl.nboxes, int(60e9 // per_box)))
+    h.hydro_ctu_step(max(1, args.warmup), batch_boxes=nb)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    n0 = h.hydro_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(h.stream)
+    h.hydro_ctu_step(args.steps, batch_boxes=nb)
+    e1.record(h.stream)
+    barrier()
+    ms_total = reduce_max(e0.elapsed_time(e1), world, dev)
+    launches = h.hydro_launch_count() - n0
+    sampler.stop_flag = True
+    sampler.join(timeout=10)
+    peak, peak_src = measured_peaks()
+    Z, nq, nvar = wl.zones, wl.nflux, wl.nvar
+    # bytes per zone of one step with every intermediate array in HBM (DESIGN.md sec. 12): trace reads the state
+    # 3 x 5 zones deep and writes 2*NQ*3; first fluxes read 2*NQ*3, write NQ*3; final fluxes read 2*NQ*3 + 4*NQ*3,
+    # write NQ*3; update reads 2*NQ*3 + NVAR, writes NVAR
+    alg = Z * 8 * (3 * nvar + 6 * nq + 6 * nq + 3 * nq + 6 * nq + 12 * nq + 3 * nq + 6 * nq + 2 * nvar)
+    ms_step = ms_total / args.steps
+    if int(os.environ.get("RANK", "0")) == 0:
+        cfg = workload_config(wl, args.config)
+        cfg.update({"integrator": "CTU (O12): PPM + characteristic tracing + 6-solve transverse corrections, one update per step",
+                    "batch_boxes": nb, "replicas": world,
+                    "call": f"hydro_ctu_step(h, scratch, {nb} boxes per batch, {args.steps} steps) -- one C-ABI call"})
+        line = {"metric": METRIC.replace("RK2", "CTU"), "value": job_value(Z, args.steps, ms_total, world), "unit": UNIT,
+                "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+                "roofline": {"bound": "hbm", "kernel": "whole CTU step (first CUDA path, intermediates in HBM)",
+                             "achieved": alg / 1e9 / (ms_step * 1e-3), "peak": peak, "unit": "GB/s",
+                             "frac": alg / 1e9 / (ms_step * 1e-3) / peak, "traffic": None, "peak_source": peak_src,
+                             "alg_bytes_per_zone_update": alg / Z},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": int(launches), "clocks": sampler.summary()}
+        print(json.dumps(line), flush=True)
+
+
 # ----------------------------------------------------------------------------- our arm
 def run_ours(args, rank, world, local_rank):
     import torch
@@ -269,6 +314,8 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    if args.ctu:
+        return run_ctu(args, wl, h, host, t_gen, barrier, local_rank, world, dev)
     h.hydro_step(args.warmup, want_dt=False)
     barrier()
     sampler = ClockSampler(local_rank)
@@ -414,6 +461,7 @@ def main():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--flatten", action="store_true", help="switch the optional shock flattening O10 on")
     ap.add_argument("--evolve", action="store_true", help="switch the optional evolved rho*e O11 on")
+    ap.add_argument("--ctu", action="store_true", help="time the CTU update O12 (hydro_ctu_step) instead of the RK2 path")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -34,15 +34,18 @@ __device__ __forceinline__ long long ctu_off(const Geom& g, int bb, int kind, in
     return ((long long)bb * 12 + kind * 3 + d) * nq * g.cstride;
 }
 
-// grid (ceil(n0/32) * nbatch, n1, n2) with n_d = nb_d + 2*ext (+1 along `face`): zone / face indices
-// lo .. of the batch box; returns false outside
+constexpr int CTU_BY = 4;      // a CTA = 32 zones along x times CTU_BY rows
+
+// block (32, CTU_BY), grid (ceil(n0/32) * nbatch, ceil(n1/CTU_BY), n2) with n_d = nb_d + 2*ext (+1 along `face`):
+// zone / face indices lo .. of the batch box; returns false outside
 __device__ __forceinline__ bool ctu_zone(const Geom& g, const int (&lo)[3], const int (&n)[3], int& bb, int (&ijk)[3])
 {
     const int xblocks = (n[0] + 31) / 32;
     bb = blockIdx.x / xblocks;
     const int i = (blockIdx.x - bb * xblocks) * 32 + threadIdx.x;
-    if (i >= n[0]) return false;
-    ijk[0] = lo[0] + i; ijk[1] = lo[1] + blockIdx.y; ijk[2] = lo[2] + blockIdx.z;
+    const int j = blockIdx.y * CTU_BY + threadIdx.y;
+    if (i >= n[0] || j >= n[1]) return false;
+    ijk[0] = lo[0] + i; ijk[1] = lo[1] + j; ijk[2] = lo[2] + blockIdx.z;
     return true;
 }
 
@@ -77,7 +80,7 @@ __device__ __forceinline__ void ctu_parabola(const double (&a)[5], double& aL, d
 
 // ---- C2-C5, hydro variables: traced states of zones -1 .. nb of every direction, along DIR ----------------------
 template <int DIR>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_trace_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
     const int lo[3] = {-1, -1, -1}, n[3] = {g.nb[0] + 2, g.nb[1] + 2, g.nb[2] + 2};
@@ -146,33 +149,35 @@ k_ctu_trace_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuArg
     }
 }
 
-// ---- C4, one species per thread (grid.y folds the species index: blockIdx.y = species * n1 + j) ----------------
+// ---- C4: all species of a zone (the five reciprocal densities of the stencil are formed once) -------------------
 template <int DIR>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_trace_species(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
-    const int n1 = g.nb[1] + 2;
-    const int s = blockIdx.y / n1;
-    const int xblocks = (g.nb[0] + 2 + 31) / 32;
-    const int bb = blockIdx.x / xblocks;
-    const int i = (blockIdx.x - bb * xblocks) * 32 + threadIdx.x;
-    if (i >= g.nb[0] + 2) return;
-    const int ijk[3] = {i - 1, (int)(blockIdx.y - s * n1) - 1, (int)blockIdx.z - 1};
+    const int lo[3] = {-1, -1, -1}, n[3] = {g.nb[0] + 2, g.nb[1] + 2, g.nb[2] + 2};
+    int bb, ijk[3];
+    if (!ctu_zone(g, lo, n, bb, ijk)) return;
     const long long z = ctu_z(g, ijk);
     const long long st = DIR == 0 ? 1 : (DIR == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
     const double* Ub = a.U + (long long)(a.box0 + bb) * g.bstride + z;
     const double dtdx = *a.dt_dev * g.dxinv[DIR];
-    double X[5], un = 0.0;
+    double rinv[5];
 #pragma unroll
-    for (int m = 0; m < 5; ++m) {
-        const double rinv = drcp(dmax(ldg(Ub + (m - 2) * st), g.small_dens));
-        X[m] = ldg(Ub + (long long)(6 + s) * g.cstride + (m - 2) * st) * rinv;
-        if (m == 2) un = ldg(Ub + (long long)(1 + DIR) * g.cstride) * rinv;
+    for (int m = 0; m < 5; ++m) rinv[m] = drcp(dmax(ldg(Ub + (m - 2) * st), g.small_dens));
+    const double un = ldg(Ub + (long long)(1 + DIR) * g.cstride) * rinv[2];
+    double* QM = a.Q + ctu_off(g, bb, 0, DIR) + z;
+    double* QP = a.Q + ctu_off(g, bb, 1, DIR) + z;
+#pragma unroll 2
+    for (int s = 0; s < g.nspec; ++s) {
+        const double* Xb = Ub + (long long)(6 + s) * g.cstride;
+        double X[5];
+#pragma unroll
+        for (int m = 0; m < 5; ++m) X[m] = ldg(Xb + (m - 2) * st) * rinv[m];
+        double aL, aR;
+        ctu_parabola(X, aL, aR);
+        QM[(long long)(5 + s) * g.cstride] = un < 0.0 ? ctu_Im(un, dtdx, X[2], aL, aR) : X[2];
+        QP[(long long)(5 + s) * g.cstride] = un > 0.0 ? ctu_Ip(un, dtdx, X[2], aL, aR) : X[2];
     }
-    double aL, aR;
-    ctu_parabola(X, aL, aR);
-    a.Q[ctu_off(g, bb, 0, DIR) + (long long)(5 + s) * g.cstride + z] = un < 0.0 ? ctu_Im(un, dtdx, X[2], aL, aR) : X[2];
-    a.Q[ctu_off(g, bb, 1, DIR) + (long long)(5 + s) * g.cstride + z] = un > 0.0 ? ctu_Ip(un, dtdx, X[2], aL, aR) : X[2];
 }
 
 // ---- C6 / C7-C9: fluxes on the low face of a zone.  FINAL = false: first fluxes from the traced states (zones
@@ -202,7 +207,7 @@ __device__ __forceinline__ void ctu_correct(const Geom& g, const CtuArgs& a, int
 }
 
 template <int DIR, bool FINAL>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_flux_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
     constexpr int E = FINAL ? 0 : 1;
@@ -228,49 +233,56 @@ k_ctu_flux_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs
     for (int c = 0; c < 5; ++c) Fo[c * g.cstride] = F[c];
 }
 
-// species fluxes F_rho * X_upwind (S7); FINAL: X of the corrected state = (rho*X)' / rho'
+// species fluxes F_rho * X_upwind (S7) of all species of a face; FINAL: X of the corrected state = (rho*X)' / rho'
 template <int DIR, bool FINAL>
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_flux_species(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
     constexpr int E = FINAL ? 0 : 1;
     int lo[3] = {-E, -E, -E}, n[3] = {g.nb[0] + 2 * E, g.nb[1] + 2 * E, g.nb[2] + 2 * E};
     lo[DIR] = 0; n[DIR] = g.nb[DIR] + 1;
-    const int s = blockIdx.y / n[1];
-    const int xblocks = (n[0] + 31) / 32;
-    const int bb = blockIdx.x / xblocks;
-    const int i = (blockIdx.x - bb * xblocks) * 32 + threadIdx.x;
-    if (i >= n[0]) return;
-    const int ijk[3] = {lo[0] + i, lo[1] + (int)(blockIdx.y - s * n[1]), lo[2] + (int)blockIdx.z};
+    int bb, ijk[3];
+    if (!ctu_zone(g, lo, n, bb, ijk)) return;
     const long long z = ctu_z(g, ijk);
     const long long st = DIR == 0 ? 1 : (DIR == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
-    const long long cs5 = (long long)(5 + s) * g.cstride;
-    double XL = a.Q[ctu_off(g, bb, 1, DIR) + cs5 + z - st];
-    double XR = a.Q[ctu_off(g, bb, 0, DIR) + cs5 + z];
-    if (FINAL) {
-        const double hdt = HALF * *a.dt_dev;
-#pragma unroll
-        for (int side = 0; side < 2; ++side) {
-            const long long zz = side ? z : z - st;
-            const double rf = a.Q[ctu_off(g, bb, side ? 0 : 1, DIR) + zz];        // traced density of the face state
-            double r = rf, rx = rf * (side ? XR : XL);
-            for (int dd = 0; dd < 3; ++dd) {
-                if (dd == DIR) continue;
-                const long long sd = dd == 0 ? 1 : (dd == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1]);
-                const double* F = a.Q + ctu_off(g, bb, 2, dd) + zz;
-                r = r - hdt * g.dxinv[dd] * (F[sd] - F[0]);
-                rx = rx - hdt * g.dxinv[dd] * (F[cs5 + sd] - F[cs5]);
-            }
-            const double X = rx * drcp(dmax(r, g.small_dens));
-            if (side) XR = X; else XL = X;
-        }
+    constexpr int D1 = DIR == 0 ? 1 : 0, D2 = DIR == 2 ? 1 : 2;       // the other two directions, ascending
+    const long long s1 = D1 == 0 ? 1 : (long long)g.nt[0];
+    const long long s2 = D2 == 1 ? (long long)g.nt[0] : (long long)g.nt[0] * g.nt[1];
+    const double* QPl = a.Q + ctu_off(g, bb, 1, DIR) + z - st;        // left state: high face of the zone below
+    const double* QMr = a.Q + ctu_off(g, bb, 0, DIR) + z;             // right state: low face of this zone
+    const double* F1a = a.Q + ctu_off(g, bb, 2, D1);
+    const double* F1b = a.Q + ctu_off(g, bb, 2, D2);
+    double* Fo = a.Q + ctu_off(g, bb, FINAL ? 3 : 2, DIR) + z;
+    const double Frho = Fo[0];
+    const double hdt = FINAL ? HALF * *a.dt_dev : 0.0;
+    double rfL = 0.0, rfR = 0.0, rinvL = 0.0, rinvR = 0.0;
+    if (FINAL) {      // corrected densities of the two face states (the expressions of ctu_correct)
+        rfL = QPl[0]; rfR = QMr[0];
+        double rL = rfL, rR = rfR;
+        rL = rL - hdt * g.dxinv[D1] * (F1a[z - st + s1] - F1a[z - st]);
+        rL = rL - hdt * g.dxinv[D2] * (F1b[z - st + s2] - F1b[z - st]);
+        rR = rR - hdt * g.dxinv[D1] * (F1a[z + s1] - F1a[z]);
+        rR = rR - hdt * g.dxinv[D2] * (F1b[z + s2] - F1b[z]);
+        rinvL = drcp(dmax(rL, g.small_dens)); rinvR = drcp(dmax(rR, g.small_dens));
     }
-    const double Frho = a.Q[ctu_off(g, bb, FINAL ? 3 : 2, DIR) + z];
-    a.Q[ctu_off(g, bb, FINAL ? 3 : 2, DIR) + cs5 + z] = Frho * (Frho >= 0.0 ? XL : XR);
+#pragma unroll 2
+    for (int s = 0; s < g.nspec; ++s) {
+        const long long cs5 = (long long)(5 + s) * g.cstride;
+        double XL = QPl[cs5], XR = QMr[cs5];
+        if (FINAL) {
+            double xl = rfL * XL, xr = rfR * XR;
+            xl = xl - hdt * g.dxinv[D1] * (F1a[cs5 + z - st + s1] - F1a[cs5 + z - st]);
+            xl = xl - hdt * g.dxinv[D2] * (F1b[cs5 + z - st + s2] - F1b[cs5 + z - st]);
+            xr = xr - hdt * g.dxinv[D1] * (F1a[cs5 + z + s1] - F1a[cs5 + z]);
+            xr = xr - hdt * g.dxinv[D2] * (F1b[cs5 + z + s2] - F1b[cs5 + z]);
+            XL = xl * rinvL; XR = xr * rinvR;
+        }
+        Fo[cs5] = Frho * (Frho >= 0.0 ? XL : XR);
+    }
 }
 
-// ---- C1 + C8 + O7: conservative update of the valid zones; grid.y folds the flux component for the species ----
-__global__ void __launch_bounds__(32)
+// ---- C1 + C8 + O7: conservative update of the valid zones ----------------------------------------------------
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_update_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
     const int lo[3] = {0, 0, 0}, n[3] = {g.nb[0], g.nb[1], g.nb[2]};
@@ -304,24 +316,25 @@ k_ctu_update_hydro(const __grid_constant__ Geom g, const __grid_constant__ CtuAr
     a.Unew[zo + 5 * g.cstride] = re;
 }
 
-__global__ void __launch_bounds__(32)
+__global__ void __launch_bounds__(32 * CTU_BY)
 k_ctu_update_species(const __grid_constant__ Geom g, const __grid_constant__ CtuArgs a)
 {
-    const int s = blockIdx.y / g.nb[1];
-    const int xblocks = (g.nb[0] + 31) / 32;
-    const int bb = blockIdx.x / xblocks;
-    const int i = (blockIdx.x - bb * xblocks) * 32 + threadIdx.x;
-    if (i >= g.nb[0]) return;
-    const int ijk[3] = {i, (int)(blockIdx.y - s * g.nb[1]), (int)blockIdx.z};
+    const int lo[3] = {0, 0, 0}, n[3] = {g.nb[0], g.nb[1], g.nb[2]};
+    int bb, ijk[3];
+    if (!ctu_zone(g, lo, n, bb, ijk)) return;
     const long long z = ctu_z(g, ijk);
     const long long st[3] = {1, g.nt[0], (long long)g.nt[0] * g.nt[1]};
-    const long long cs5 = (long long)(5 + s) * g.cstride;
-    const double* F0 = a.Q + ctu_off(g, bb, 3, 0) + cs5 + z;
-    const double* F1 = a.Q + ctu_off(g, bb, 3, 1) + cs5 + z;
-    const double* F2 = a.Q + ctu_off(g, bb, 3, 2) + cs5 + z;
-    const double L = -(F0[st[0]] - F0[0]) * g.dxinv[0] - (F1[st[1]] - F1[0]) * g.dxinv[1] - (F2[st[2]] - F2[0]) * g.dxinv[2];
-    const long long zo = (long long)(a.box0 + bb) * g.bstride + (long long)(6 + s) * g.cstride + z;
-    a.Unew[zo] = a.U[zo] + *a.dt_dev * L;
+    const double dt = *a.dt_dev;
+#pragma unroll 2
+    for (int s = 0; s < g.nspec; ++s) {
+        const long long cs5 = (long long)(5 + s) * g.cstride;
+        const double* F0 = a.Q + ctu_off(g, bb, 3, 0) + cs5 + z;
+        const double* F1 = a.Q + ctu_off(g, bb, 3, 1) + cs5 + z;
+        const double* F2 = a.Q + ctu_off(g, bb, 3, 2) + cs5 + z;
+        const double L = -(F0[st[0]] - F0[0]) * g.dxinv[0] - (F1[st[1]] - F1[0]) * g.dxinv[1] - (F2[st[2]] - F2[0]) * g.dxinv[2];
+        const long long zo = (long long)(a.box0 + bb) * g.bstride + (long long)(6 + s) * g.cstride + z;
+        a.Unew[zo] = a.U[zo] + dt * L;
+    }
 }
 
 }  // namespace hydro

@@ -641,23 +641,24 @@ int ctu_dir(hydro_handle h, const CtuArgs &a, int phase)
 {
     const Geom &g = h->g;
     const int nb[3] = {g.nb[0], g.nb[1], g.nb[2]};
-    auto grid = [&](int ext, int face, int ncomp) {
+    auto grid = [&](int ext, int face) {
         int n[3] = {nb[0] + 2 * ext, nb[1] + 2 * ext, nb[2] + 2 * ext};
         if (face >= 0) n[face] = nb[face] + 1;
-        return dim3((unsigned)(((n[0] + 31) / 32) * a.nbatch), (unsigned)(n[1] * ncomp), (unsigned)n[2]);
+        return dim3((unsigned)(((n[0] + 31) / 32) * a.nbatch), (unsigned)((n[1] + CTU_BY - 1) / CTU_BY), (unsigned)n[2]);
     };
+    const dim3 blk(32, CTU_BY);
     int rc = HYDRO_OK;
     const int ns = g.nspec;
     prof_begin(h);
-    if (phase == 0) k_ctu_trace_hydro<DIR><<<grid(1, -1, 1), 32, 0, h->stream>>>(g, a);
-    else if (phase == 1) k_ctu_flux_hydro<DIR, false><<<grid(1, DIR, 1), 32, 0, h->stream>>>(g, a);
-    else k_ctu_flux_hydro<DIR, true><<<grid(0, DIR, 1), 32, 0, h->stream>>>(g, a);
+    if (phase == 0) k_ctu_trace_hydro<DIR><<<grid(1, -1), blk, 0, h->stream>>>(g, a);
+    else if (phase == 1) k_ctu_flux_hydro<DIR, false><<<grid(1, DIR), blk, 0, h->stream>>>(g, a);
+    else k_ctu_flux_hydro<DIR, true><<<grid(0, DIR), blk, 0, h->stream>>>(g, a);
     if ((rc = check_launch(h, "k_ctu hydro", K_CTU))) return rc;
     if (ns > 0) {
         prof_begin(h);
-        if (phase == 0) k_ctu_trace_species<DIR><<<grid(1, -1, ns), 32, 0, h->stream>>>(g, a);
-        else if (phase == 1) k_ctu_flux_species<DIR, false><<<grid(1, DIR, ns), 32, 0, h->stream>>>(g, a);
-        else k_ctu_flux_species<DIR, true><<<grid(0, DIR, ns), 32, 0, h->stream>>>(g, a);
+        if (phase == 0) k_ctu_trace_species<DIR><<<grid(1, -1), blk, 0, h->stream>>>(g, a);
+        else if (phase == 1) k_ctu_flux_species<DIR, false><<<grid(1, DIR), blk, 0, h->stream>>>(g, a);
+        else k_ctu_flux_species<DIR, true><<<grid(0, DIR), blk, 0, h->stream>>>(g, a);
         rc = check_launch(h, "k_ctu species", K_CTU);
     }
     return rc;
@@ -682,11 +683,12 @@ int ctu_chunk(hydro_handle h, char *scratch, size_t bytes, int nsteps, double *d
                 if ((rc = ctu_dir<2>(h, a, phase))) return rc;
             }
             prof_begin(h);
-            k_ctu_update_hydro<<<dim3((unsigned)(((g.nb[0] + 31) / 32) * a.nbatch), g.nb[1], g.nb[2]), 32, 0, h->stream>>>(g, a);
+            const dim3 ugrid((unsigned)(((g.nb[0] + 31) / 32) * a.nbatch), (unsigned)((g.nb[1] + CTU_BY - 1) / CTU_BY), g.nb[2]);
+            k_ctu_update_hydro<<<ugrid, dim3(32, CTU_BY), 0, h->stream>>>(g, a);
             if ((rc = check_launch(h, "k_ctu_update_hydro", K_CTU))) return rc;
             if (g.nspec > 0) {
                 prof_begin(h);
-                k_ctu_update_species<<<dim3((unsigned)(((g.nb[0] + 31) / 32) * a.nbatch), g.nb[1] * g.nspec, g.nb[2]), 32, 0, h->stream>>>(g, a);
+                k_ctu_update_species<<<ugrid, dim3(32, CTU_BY), 0, h->stream>>>(g, a);
                 if ((rc = check_launch(h, "k_ctu_update_species", K_CTU))) return rc;
             }
         }
@@ -933,8 +935,8 @@ int hydro_ctu_step(hydro_handle h, void *ctu_scratch_dev, size_t ctu_scratch_byt
     if (h->external) return fail(h, HYDRO_EINVAL, "hydro_ctu_step cannot run on a shard (HYDRO_BC_EXTERNAL)");
     if (!ctu_scratch_dev || ((uintptr_t)ctu_scratch_dev & 15)) return fail(h, HYDRO_EINVAL, "null or misaligned CTU scratch");
     if (ctu_scratch_bytes < ctu_box_bytes(g)) return fail(h, HYDRO_ENOMEM, "ctu_scratch_bytes too small (hydro_ctu_scratch_bytes)");
-    if ((long long)(g.nb[1] + 2) * (g.nspec > 0 ? g.nspec : 1) > 65535 || g.nb[2] + 2 > 65535)
-        return fail(h, HYDRO_EINVAL, "CTU grid too large (nbox[1] * nspec or nbox[2])");
+    if (g.nb[2] + 2 > 65535 || (g.nb[1] + 2 + CTU_BY - 1) / CTU_BY > 65535)
+        return fail(h, HYDRO_EINVAL, "CTU grid too large (nbox[1] or nbox[2])");
     DeviceGuard guard(h->device);
     int cur = 0, rc = HYDRO_OK;
     for (int done = 0; done < nsteps && rc == HYDRO_OK; done += DT_SLOTS) {

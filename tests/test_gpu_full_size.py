@@ -44,7 +44,7 @@ def device_window(wl, h, lo, n):
     return out
 
 
-def check_windows(wl, h, dt, windows, size=40, tol=1e-11):
+def check_windows(wl, h, dt, windows, size=40, tol=1e-11, stepper=None):
     """windows: list of (x,y,z) anchors; an anchor component of None on an axis = flush with the low
     domain boundary (real BC there), 'hi' = flush with the high boundary.
     dt: the GPU's dt of the one step taken, or the list of its dts of the n steps taken (the oracle advances the
@@ -83,7 +83,7 @@ def check_windows(wl, h, dt, windows, size=40, tol=1e-11):
         U0 = W.scatter_valid(sub, G0)
         U1 = np.zeros_like(U0)
         for dt_s in dts:
-            O.step_fixed_dt(O.make_params(sub.params), U0, U1, dt_s)
+            (stepper or O.step_fixed_dt)(O.make_params(sub.params), U0, U1, dt_s)
         Go = W.gather_valid(sub, U0)
         Gg = device_window(wl, h, lo, n)
         sl = (slice(None),) + tuple(slice(*keep[d]) for d in (2, 1, 0))
@@ -175,6 +175,21 @@ def test_config3_ten_steps_in_one_call():
     dts = h.hydro_step(10, all_dts=True)                             # BASELINE config 3: 10 steps
     worst = check_windows(wl, h, dts, [(20, 52, 84), (180, 180, 180)], size=160, tol=1e-10)
     print("config 3, 10 steps: worst window error", worst)
+
+
+def test_config3_ten_ctu_steps_in_one_call():
+    """The CTU update O12 at a BASELINE size: config 3 (256^3, 64 boxes), 10 steps in one hydro_ctu_step call, the
+    boxes in batches of 24 (ragged last batch), against oracle_ctu_step on windows."""
+    wl, U0, h = full_run(3)
+    del U0
+    t0 = np.array(h.hydro_conserved_totals(0))
+    dts = h.hydro_ctu_step(10, batch_boxes=24, all_dts=True)
+    worst = check_windows(wl, h, dts, [(20, 52, 84), (180, 180, 180)], size=160, tol=1e-10, stepper=O.ctu_step_fixed_dt)
+    print("config 3, 10 CTU steps: worst window error", worst)
+    t1 = np.array(h.hydro_conserved_totals(0))
+    absU = h.U0.view(wl.state_shape)[:, :, 4:-4, 4:-4, 4:-4].abs().sum(dim=(0, 2, 3, 4)).cpu().numpy() * np.prod(wl.dx)
+    scale = np.array([absU[c if c < 5 else c + 1] for c in range(wl.nflux)])
+    assert np.all(np.abs(t1 - t0) <= 1e-13 * scale)
 
 
 def test_config4_atmosphere_sampled_windows():
