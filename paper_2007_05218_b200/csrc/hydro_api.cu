@@ -531,14 +531,19 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     } else {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
-        const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS) * g.nboxes;
+        const bool fold = g.nboxes > 65535;             // the box index in blockIdx.z when it fits
+        const long long gx = (long long)nchunk * ((g.nb[1] + WARPS - 1) / WARPS) * (fold ? g.nboxes : 1);
         if (gx > 2147483647LL || g.nb[2] > 65535) return fail(h, HYDRO_EINVAL, "x-sweep grid too large");
         prof_begin(h);
-        const dim3 xg((unsigned)gx, g.nb[2], 1);
-        if (g.flatten && g.evolve) k_sweep_x<WARPS, true, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
-        else if (g.flatten) k_sweep_x<WARPS, true, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
-        else if (g.evolve) k_sweep_x<WARPS, false, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
-        else k_sweep_x<WARPS, false, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
+        const dim3 xg((unsigned)gx, g.nb[2], fold ? 1 : g.nboxes);
+#define XSWEEP(FL, EV, PTR) \
+        do { if (fold) k_sweep_x<WARPS, FL, EV, true><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, PTR); \
+             else k_sweep_x<WARPS, FL, EV, false><<<xg, WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, PTR); } while (0)
+        if (g.flatten && g.evolve) XSWEEP(true, true, a.FL);
+        else if (g.flatten) XSWEEP(true, false, a.FL);
+        else if (g.evolve) XSWEEP(false, true, nullptr);
+        else XSWEEP(false, false, nullptr);
+#undef XSWEEP
         int rc = check_launch(h, "k_sweep_x", K_SWEEP_X);
         if (rc) return rc;
     }

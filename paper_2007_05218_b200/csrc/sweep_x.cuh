@@ -43,19 +43,26 @@ __device__ __forceinline__ void ppm_lanes(double a, double f, double omf, double
     qRf = shfl_dn1(aL);                                // lanes 2..28
 }
 
-template <int WARPS, bool FLAT, bool EVOLVE>
+template <int WARPS, bool FLAT, bool EVOLVE, bool FOLDB = false>
 __global__ void __launch_bounds__(WARPS * 32)
 k_sweep_x(const __grid_constant__ Geom g, const double* __restrict__ U, double* __restrict__ Lacc,
           const double* __restrict__ FL)
 {
     const int lane = threadIdx.x & 31;
     const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
-    // grid (nchunk * ceil(nb_y / WARPS) * boxes, nb_z): the chunks of a row are consecutive blocks, the
-    // warps of a block are WARPS consecutive rows; two 32-bit divisions per warp (a flat 64-bit warp
-    // index cost ~150 instructions of division per warp, 8 % of the kernel)
-    const int per_box = gridDim.x / g.nboxes;
-    const int b = blockIdx.x / per_box;
-    const int rb = blockIdx.x - b * per_box;
+    // grid (nchunk * ceil(nb_y / WARPS), nb_z, boxes): the chunks of a row are consecutive blocks, the
+    // warps of a block are WARPS consecutive rows; one 32-bit division per warp (a flat 64-bit warp
+    // index cost ~150 instructions of division per warp, 8 % of the kernel).  FOLDB (more than 65535
+    // boxes): the box index rides in blockIdx.x too, at the price of two more divisions per warp.
+    int b, rb;
+    if (FOLDB) {
+        const int per_box = gridDim.x / g.nboxes;
+        b = blockIdx.x / per_box;
+        rb = blockIdx.x - b * per_box;
+    } else {
+        b = blockIdx.z;
+        rb = blockIdx.x;
+    }
     const int jb = rb / nchunk;
     const int chunk = rb - jb * nchunk;
     const int j = jb * WARPS + (threadIdx.x >> 5);

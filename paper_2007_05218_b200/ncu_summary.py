@@ -21,13 +21,18 @@ CSRC = os.path.join(HERE, "csrc")
 N_SM = 148
 
 
+# the kernel sources of the RK2 path's default launches (the classes of hydro_profile_read 0..8)
+PATH_SOURCES = ["flatten.cuh", "ghost_reduce.cuh", "hydro_device.cuh", "march_ring.cuh", "sweep_x.cuh", "sweep_yz.cuh"]
+
+
 def source_sha() -> str:
-    """SHA-256 over the CUDA sources of libhydro_b200.so (names and contents, sorted)."""
+    """SHA-256 over the kernel sources of the RK2 path (names and contents): a capture is trusted while the
+    kernels it measured are the kernels that run.  The optional paths (march_x.cuh, ctu.cuh) and the host code
+    are not part of it."""
     h = hashlib.sha256()
-    for name in sorted(os.listdir(CSRC)):
-        if name.endswith((".cu", ".cuh")) and name != "fp64_probe.cu":
-            h.update(name.encode())
-            h.update(open(os.path.join(CSRC, name), "rb").read())
+    for name in PATH_SOURCES:
+        h.update(name.encode())
+        h.update(open(os.path.join(CSRC, name), "rb").read())
     return h.hexdigest()
 
 

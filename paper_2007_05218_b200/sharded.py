@@ -81,19 +81,21 @@ def exchange_dim(dim, nbrs, pack, unpack, sendrecv):
         unpack(dim, side, buf)
 
 
-def dist_sendrecv(like):
-    """sendrecv over torch.distributed point-to-point operations (one batch per call)."""
+def dist_sendrecv(like, stage_on_host=False):
+    """sendrecv over torch.distributed point-to-point operations (one batch per call).  stage_on_host: copy the
+    buffers through host memory (for the gloo backend, which moves host tensors; NCCL sends device buffers)."""
     import torch
     import torch.distributed as dist
 
     def f(sends, recvs):
-        outs = [torch.empty_like(like(src, tag)) for src, tag in recvs]
-        ops = [dist.P2POp(dist.isend, buf, dst, tag=tag) for buf, dst, tag in sends]
+        dev = [like(src, tag) for src, tag in recvs]
+        outs = [torch.empty_like(d, device="cpu" if stage_on_host else d.device) for d in dev]
+        ops = [dist.P2POp(dist.isend, buf.cpu() if stage_on_host else buf, dst, tag=tag) for buf, dst, tag in sends]
         ops += [dist.P2POp(dist.irecv, out, src, tag=tag) for out, (src, tag) in zip(outs, recvs)]
         if ops:
             for req in dist.batch_isend_irecv(ops):
                 req.wait()
-        return outs
+        return [o.to(d.device) for o, d in zip(outs, dev)] if stage_on_host else outs
     return f
 
 
@@ -126,8 +128,9 @@ class ShardedHydro:
     def __init__(self, params: dict, pgrid, device):
         import torch.distributed as dist
         self.dist = dist
+        self.on_host = dist.get_backend() == "gloo"            # gloo: buffers and scalars go through host memory
         self.shard = Shard(params, pgrid, dist.get_rank(), device=device)
-        self.sendrecv = dist_sendrecv(lambda src, tag: self.shard.bufs[(tag // 2, tag % 2)])
+        self.sendrecv = dist_sendrecv(lambda src, tag: self.shard.bufs[(tag // 2, tag % 2)], stage_on_host=self.on_host)
 
     def fill(self, which):
         s = self.shard
@@ -139,7 +142,7 @@ class ShardedHydro:
     def step(self):
         import torch
         s = self.shard
-        dt = torch.tensor([s.h.hydro_estimate_dt()], dtype=torch.float64, device=s.h.device)
+        dt = torch.tensor([s.h.hydro_estimate_dt()], dtype=torch.float64, device="cpu" if self.on_host else s.h.device)
         self.dist.all_reduce(dt, op=self.dist.ReduceOp.MIN)          # the one collective of a step: 8 bytes
         dt = float(dt.item())
         self.fill(0)
@@ -150,7 +153,8 @@ class ShardedHydro:
 
     def totals(self):
         import torch
-        t = torch.tensor(self.shard.h.hydro_conserved_totals(0), dtype=torch.float64, device=self.shard.h.device)
+        t = torch.tensor(self.shard.h.hydro_conserved_totals(0), dtype=torch.float64,
+                         device="cpu" if self.on_host else self.shard.h.device)
         self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
         return t.tolist()
 

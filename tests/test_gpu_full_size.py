@@ -258,3 +258,26 @@ def test_config3_evolve_and_flatten_are_noops_on_subsonic_smooth_flow():
     A, B = h.U0.view(wl.state_shape), h2.U0.view(wl.state_shape)
     for b in range(wl.nboxes):
         assert torch.equal(A[b, :, ng:-ng, ng:-ng, ng:-ng], B[b, :, ng:-ng, ng:-ng, ng:-ng]), b
+
+
+def test_more_than_65535_boxes():
+    """2048 x 2048 x 8 zones in 65 536 boxes of 8^3 (the box index rides in blockIdx.x everywhere, k_sweep_x in its
+    FOLDB form): two steps through hydro_step must equal, bit for bit, the same state cut into 1 024 boxes of
+    64 x 64 x 8 (decomposition invariance, pin P8, which the oracle tests pin on the CPU)."""
+    import torch
+    from paper_2007_05218_b200.binding import Hydro
+    small = W.config(3, ndom=(2048, 2048, 8), nbox=(8, 8, 8), nspec=1)
+    big = W.config(3, ndom=(2048, 2048, 8), nbox=(64, 64, 8), nspec=1)
+    assert small.nboxes == 65536
+    prim = W.primitives(big, (0, 0, 0), (8, 2048, 2048))
+    G0 = W.conserved_from_primitives(big.params["gamma"], *prim)
+    out = []
+    for wl in (small, big):
+        h = Hydro(wl.params)
+        h.upload(W.scatter_valid(wl, G0), 0)
+        dts = h.hydro_step(2, all_dts=True)
+        out.append((dts, W.gather_valid(wl, h.download(0).reshape(wl.state_shape))))
+        del h
+        torch.cuda.empty_cache()
+    assert out[0][0] == out[1][0]
+    assert np.array_equal(out[0][1], out[1][1])
