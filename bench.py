@@ -46,7 +46,7 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt, xmarch=False):
+def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt, xmarch=False, one_launch=0):
     """Algorithmic HBM bytes per launch of each kernel class: what the kernel
     split must move -- every input once with the 3-zone PPM halo along the sweep direction, every
     output once.  Returns {class: mean bytes per launch over the launches of `steps` steps issued
@@ -105,6 +105,13 @@ def algorithmic_bytes(wl, ns_groups, steps, split_ghosts, fuse_dt, xmarch=False)
             sz.append(Z * (2 * 8 * halo[2] + 8 * face[2] + 4 * 8 + 8 * (1 + xend) + 0.5 * 8 + (8 * halo[2] if fl else 0)))
         out["species_y"] = float(np.mean(sy))
         out["species_z"] = float(np.mean(sz))
+        # all groups in one launch (hydro_query 5): the launch reads rho (with its halo) and F_rho once, not once per group
+        shared = [Z * (8 * halo[d] + 8 * face[d]) for d in (1, 2)]
+        n_sp = len(groups)            # the O11 energy launch stays a launch of its own
+        if one_launch & 1 and n_sp >= 2:
+            out["species_y"] = (float(np.sum(sy[:n_sp])) - (n_sp - 1) * shared[0] + float(np.sum(sy[n_sp:]))) / (1 + len(sy) - n_sp)
+        if one_launch & 2 and n_sp >= 2:
+            out["species_z"] = (float(np.sum(sz[:n_sp])) - (n_sp - 1) * shared[1] + float(np.sum(sz[n_sp:]))) / (1 + len(sz) - n_sp)
     return out
 
 
@@ -323,6 +330,7 @@ def run_ours(args, rank, world, local_rank):
     launches0 = h.hydro_launch_count()
     ns_max, split_ghosts, fuse_dt = h.hydro_query(3), bool(h.hydro_query(1)), bool(h.hydro_query(2))
     xmarch = bool(h.hydro_query(4))
+    one_launch = max(0, h.hydro_query(5))
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(h.stream)
@@ -348,7 +356,7 @@ def run_ours(args, rank, world, local_rank):
     peak, peak_src = measured_peaks()
     ngroups = max(1, -(-wl.nspec // ns_max)) if wl.nspec else 0
     groups = [wl.nspec // ngroups + (1 if i < wl.nspec % ngroups else 0) for i in range(ngroups)] if ngroups else []
-    alg = algorithmic_bytes(wl, groups, args.steps, split_ghosts, fuse_dt, xmarch)
+    alg = algorithmic_bytes(wl, groups, args.steps, split_ghosts, fuse_dt, xmarch, one_launch)
     kernels = {}
     tot_ms = sum(v[0] for v in prof.values())
     for k, (ms, cnt) in prof.items():
@@ -438,7 +446,7 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         cfg = workload_config(wl, args.config)
         cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
-                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt, "x_sweep": "marching (march_x.cuh)" if xmarch else "lane-parallel (sweep_x.cuh)",
+                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt, "x_sweep": "marching (march_x.cuh)" if xmarch else "lane-parallel (sweep_x.cuh)", "species_groups_in_one_launch": {"y": bool(one_launch & 1), "z": bool(one_launch & 2)},
                     "call": f"hydro_step(h, {args.steps}) -- one C-ABI call for the K timed steps",
                     "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

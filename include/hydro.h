@@ -99,6 +99,8 @@ size_t hydro_scratch_bytes(const hydro_params *p);
  *                           lane-parallel k_sweep_x (measured equal in time, profiles/r02_xmarch.md)  [0]
  *   HYDRO_SEGLEN=n          zones per pencil segment of the y/z sweeps                       [auto]
  *   HYDRO_NSMAX=n           passive species per thread and launch, 1..5                      [5]
+ *   HYDRO_SPECIES_ONE_LAUNCH=m  bit 0: the y species sweep, bit 1: the z species sweep launches all species groups
+ *                           together (sibling CTAs share rho and F_rho rows through L2) instead of one by one     [1]
  *   HYDRO_FUSE_DT=0         hydro_step runs k_estimate_dt every step                         [1]
  *   HYDRO_SPLIT_GHOSTS=0    hydro_step / hydro_fill_ghosts use the one-launch ghost fill     [1]
  *   HYDRO_FILL_MONOLITHIC=1 hydro_fill_ghosts alone uses the one-launch ghost fill           [0] */
@@ -172,7 +174,8 @@ int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *
  *        2: hydro_step reduces the next step's dt inside the stage-1 z hydro sweep;
  *        3: passive species per thread and launch in the species sweeps;
  *        4: the x sweep runs as marching kernels (a thread per row, march_x.cuh; 1) or as the
- *           lane-parallel k_sweep_x (0).
+ *           lane-parallel k_sweep_x (0);
+ *        5: which species sweeps launch all species groups together (bit 0: y, bit 1: z).
  * Returns -1 for a NULL handle or an unknown `what`. */
 int hydro_query(hydro_handle h, int what);
 

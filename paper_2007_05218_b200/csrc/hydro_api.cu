@@ -55,7 +55,7 @@ struct Carve {
 
 // tuning switches, read from the environment ONCE per hydro_init (include/hydro.h lists them)
 struct Knobs {
-    int ring, seglen, nsmax, fuse_dt, split_ghosts, fill_monolithic, xmarch;
+    int ring, seglen, nsmax, fuse_dt, split_ghosts, fill_monolithic, xmarch, species_one_launch;
 };
 
 int env_int(const char *name, int dflt)
@@ -343,6 +343,31 @@ void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, 
     }
 }
 
+// all species groups of a direction in ONE launch (k_march_species_groups): nsa = species of the larger groups
+template <int DIR, bool FINAL, int STAGE>
+void launch_species_groups(hydro_handle h, const SweepArgs &a, int nsa, dim3 grid, int state)
+{
+    RingMaps tm;
+    tm.a = h->maps[state][DIR - 1][1];
+    tm.b = h->maps[state][DIR - 1][nsa];
+    tm.b2 = h->maps[state][DIR - 1][nsa > 1 ? nsa - 1 : 1];
+    tm.f = h->fmaps[DIR - 1];
+    const bool flat = h->g.flatten != 0;
+    const size_t sm = (size_t)RING_D * (1 + nsa + (flat ? 1 : 0)) * BS * 8 + RING_D * 8;
+    grid.x *= a.ngroups;
+    switch (nsa) {
+#define CASE(N) case N: \
+        if (flat) { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, RING_D, true>; set_smem(h, kern, sm); \
+                    kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } \
+        else { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, RING_D, false>; set_smem(h, kern, sm); \
+               kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } \
+        break;
+        CASE(2) CASE(3) CASE(4) CASE(5)
+#undef CASE
+        default: break;
+    }
+}
+
 template <int DIR, bool FINAL, int STAGE, bool FLAT, bool EVOLVE>
 void launch_hydro_ring(hydro_handle h, const SweepArgs &a, dim3 grid, int state)
 {
@@ -393,8 +418,18 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
         k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
     if (rc) return rc;
-    if (g.nspec > 0) {
-        const int ngroups = (g.nspec + h->ns_max - 1) / h->ns_max;
+    const int ngroups = g.nspec > 0 ? (g.nspec + h->ns_max - 1) / h->ns_max : 0;
+    if (ring && ngroups >= 2 && (h->kn.species_one_launch & (DIR == 1 ? 1 : 2)) && (long long)grid.x * ngroups <= 2147483647LL) {
+        // every group in one launch: sibling CTAs share their rho and F_rho rows through L2
+        const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
+        a.sbase = 0;
+        a.lacc_shift = 0;
+        a.ngroups = ngroups;
+        a.n_hi = rem > 0 ? rem : ngroups;
+        prof_begin(h);
+        launch_species_groups<DIR, FINAL, STAGE>(h, a, rem > 0 ? base + 1 : base, grid, state);
+        if ((rc = check_launch(h, "k_march_species_groups", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
+    } else if (g.nspec > 0) {
         const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
         int s0 = 0;
         for (int gr = 0; gr < ngroups; ++gr) {
@@ -763,6 +798,7 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     h->kn.split_ghosts = env_int("HYDRO_SPLIT_GHOSTS", 1);
     h->kn.fill_monolithic = env_int("HYDRO_FILL_MONOLITHIC", 0);
     h->kn.xmarch = env_int("HYDRO_XMARCH", 0);
+    h->kn.species_one_launch = env_int("HYDRO_SPECIES_ONE_LAUNCH", 1);
     h->ns_max = (h->kn.nsmax >= 1 && h->kn.nsmax <= NS_MAX) ? h->kn.nsmax : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d, h->kn.seglen);
     {   // TMA tensor copies: 16-byte row pitch AND 16-byte aligned box starts (the first valid zone of a row sits
@@ -965,6 +1001,7 @@ int hydro_query(hydro_handle h, int what)
         case 2: return h->fuse_dt ? 1 : 0;
         case 3: return h->ns_max;
         case 4: return h->use_xmarch ? 1 : 0;
+        case 5: return h->use_ring ? (h->kn.species_one_launch & 3) : 0;
         default: return -1;
     }
 }

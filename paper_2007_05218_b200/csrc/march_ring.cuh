@@ -88,7 +88,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 // The two tensor maps of a launch (built on the host, hydro_api.cu): `a` and `b` view the
 // stage state with boxes {W, R rows, NCa components} and {W, R rows, NCb components}.
 struct RingMaps {
-    CUtensorMap a, b;
+    CUtensorMap a, b, b2;
     CUtensorMap f;       // flattening coefficients (FLAT kernels): {W, R rows, 1} boxes of the FL array
 };
 
@@ -380,9 +380,11 @@ k_march_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 // sbase+NS-1 (map b, NS components).
 // ENERGY (NS = 1, FINAL, launched with sbase = -1): the one "species" is e = rho*e / rho of O11; the update adds
 // -p div(u_face) and ends with the dual-energy switch (readings G3-G5).
-template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT, bool ENERGY = false>
-__global__ void __launch_bounds__(BS, RING_MINB_S)
-k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
+// The march of one CTA: bx / gx = this CTA's index and the CTA count of ITS species group along grid.x
+// ((CTAs per box) * boxes), sbase = first species of the group, mapb = tensor map with NS-component boxes.
+template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT, bool ENERGY>
+__device__ __forceinline__ void march_species_body(const Geom& g, const SweepArgs& a, const CUtensorMap* mapa,
+                                                   const CUtensorMap* mapb, const CUtensorMap* mapf, int bx, int gx, int sbase)
 {
     constexpr int ROW_F = 1 + NS;             // ring row of the flattening coefficient (FLAT)
     constexpr int NROW = ROW_F + (FLAT ? 1 : 0);
@@ -392,13 +394,12 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
 
     const int tid = threadIdx.x;
-    const int tiles = gridDim.x / g.nboxes;      // grid.x = (CTAs per box) * boxes
-    const int b = blockIdx.x / tiles;
-    const RingMap m = ring_map<DIR, BS>(g, tid, blockIdx.x - b * tiles);
+    const int tiles = gx / g.nboxes;
+    const int b = bx / tiles;
+    const RingMap m = ring_map<DIR, BS>(g, tid, bx - b * tiles);
     const int m0 = blockIdx.y * a.seglen;
     const int m1 = min(m0 + a.seglen, g.nb[DIR]);
     const int nsteps = m1 - m0 + 6;
-    const int sbase = a.sbase;
     const long long mstride = (DIR == 1) ? g.nt[0] : (long long)g.nt[0] * g.nt[1];
     const long long lmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
 
@@ -406,15 +407,15 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         uint64_t* bar = &full[it % D];
         double* slot = ring + (size_t)(it % D) * NROW * BS;
         mbar_expect_tx(bar, (uint32_t)(NROW * BS * 8));
-        ring_issue<DIR>(g, m, &tm.a, slot, bar, m0 - 3 + it, 0, b);
-        ring_issue<DIR>(g, m, &tm.b, slot + BS, bar, m0 - 3 + it, 6 + sbase, b);
-        if (FLAT) ring_issue<DIR>(g, m, &tm.f, slot + ROW_F * BS, bar, m0 - 3 + it, 0, b);
+        ring_issue<DIR>(g, m, mapa, slot, bar, m0 - 3 + it, 0, b);
+        ring_issue<DIR>(g, m, mapb, slot + BS, bar, m0 - 3 + it, 6 + sbase, b);
+        if (FLAT) ring_issue<DIR>(g, m, mapf, slot + ROW_F * BS, bar, m0 - 3 + it, 0, b);
     };
 
     if (tid == 0) {
-        tma_prefetch_desc(&tm.a);
-        tma_prefetch_desc(&tm.b);
-        if (FLAT) tma_prefetch_desc(&tm.f);
+        tma_prefetch_desc(mapa);
+        tma_prefetch_desc(mapb);
+        if (FLAT) tma_prefetch_desc(mapf);
         for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
@@ -520,6 +521,32 @@ k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
         }
         __syncthreads();
         if (tid == 0 && it >= KEEP && it - KEEP + D < nsteps) issue(it - KEEP + D);
+    }
+}
+
+// One species group per launch (also the O11 energy launch: ENERGY, NS = 1, sbase = -1).
+template <int DIR, bool FINAL, int STAGE, int NS, int BS, int D, bool FLAT, bool ENERGY = false>
+__global__ void __launch_bounds__(BS, RING_MINB_S)
+k_march_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
+{
+    march_species_body<DIR, FINAL, STAGE, NS, BS, D, FLAT, ENERGY>(g, a, &tm.a, &tm.b, &tm.f, blockIdx.x, gridDim.x, a.sbase);
+}
+
+// ALL species groups in one launch: CTA blockIdx.x works on group blockIdx.x % ngroups of tile blockIdx.x / ngroups,
+// so that the CTAs which read the same rho and F_rho rows are dispatched together and march in step -- the rows one
+// of them pulls from HBM are L2 hits for its siblings (the groups re-read rho and F_rho: 16 B per zone and group).
+// The first a.n_hi groups carry NSA species, the others NSA - 1 (maps tm.b / tm.b2); CTA-uniform branch.
+template <int DIR, bool FINAL, int STAGE, int NSA, int BS, int D, bool FLAT>
+__global__ void __launch_bounds__(BS, RING_MINB_S)
+k_march_species_groups(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a, const __grid_constant__ RingMaps tm)
+{
+    const int group = blockIdx.x % a.ngroups, bx = blockIdx.x / a.ngroups, gx = gridDim.x / a.ngroups;
+    if (group < a.n_hi) {
+        march_species_body<DIR, FINAL, STAGE, NSA, BS, D, FLAT, false>(g, a, &tm.a, &tm.b, &tm.f, bx, gx, group * NSA);
+    } else {
+        constexpr int NSB = NSA > 1 ? NSA - 1 : 1;
+        march_species_body<DIR, FINAL, STAGE, NSB, BS, D, FLAT, false>(g, a, &tm.a, &tm.b2, &tm.f, bx, gx,
+                                                                      a.n_hi * NSA + (group - a.n_hi) * NSB);
     }
 }
 

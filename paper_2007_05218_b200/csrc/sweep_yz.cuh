@@ -34,6 +34,7 @@ struct SweepArgs {
     unsigned long long* red;
     double* dt_next;
     const double* FL;      // O10 flattening coefficients (padded, one array per box) or nullptr
+    int ngroups, n_hi;     // k_march_species_groups: species groups in the launch, and how many carry the larger count
     int lacc_shift;        // species kernels: accumulator component = 5 + sbase + lacc_shift (0 for species; the
                            // O11 energy launch uses sbase = -1, i.e. state component 5, and the slot after the fluxes)
 };
