@@ -38,7 +38,7 @@ def source_sha() -> str:
 
 def classify(kernel: str):
     """kernel name -> (class of hydro_profile_read, stage or None)."""
-    m = re.search(r"k_march_(hydro|species)<(\d), *(\d), *(\d)", kernel)
+    m = re.search(r"k_march_(hydro|species)(?:_groups)?<(\d), *(\d), *(\d)", kernel)
     if m:
         return f"{m.group(1)}_{'y' if m.group(2) == '1' else 'z'}", (int(m.group(4)) if m.group(3) == "1" else None)
     m = re.search(r"k_sweep_(hydro|species)<(\d), *(\d), *(\d)", kernel)
@@ -140,12 +140,12 @@ def main():
             f.write(f"# {a.title}\n\nCommand (committed files only):\n\n```\n{a.command}\n```\n\n")
             f.write("`TB/s` = (DRAM read + write) / duration under ncu (clocks not locked, kernels serialised, cold cache).  "
                     f"Sources: sha256 {source_sha()[:16]}.\n\n")
-            f.write("| # | kernel | ms | rd GB | wr GB | TB/s | dram % | fp64 % | issue % | warps % | regs | warp instr | top stalls |\n")
-            f.write("|---|---|---|---|---|---|---|---|---|---|---|---|---|\n")
+            f.write("| # | kernel | ms | rd GB | wr GB | TB/s | fp64 % | issue % | warps % | regs | warp instr | top stalls |\n")
+            f.write("|---|---|---|---|---|---|---|---|---|---|---|---|\n")
             for i, L in enumerate(launches):
                 tb = (L["dram_read"] + L["dram_write"]) / 1e12 / (L["ms"] * 1e-3)
                 f.write(f"| {i} | `{L['kernel']}` | {L['ms']:.3f} | {L['dram_read'] / 1e9:.2f} | {L['dram_write'] / 1e9:.2f} | {tb:.2f} | "
-                        f"{L['dram_pct']:.1f} | {L['fp64_pct']:.1f} | {L['issue_pct']:.1f} | {L['warps_pct']:.1f} | {L['regs']:.0f} | "
+                        f"{L['fp64_pct']:.1f} | {L['issue_pct']:.1f} | {L['warps_pct']:.1f} | {L['regs']:.0f} | "
                         f"{L['warp_instr']:.3g} | {', '.join(L['stalls'])} |\n")
             tot_ms = sum(L["ms"] for L in launches)
             tot_b = sum(L["dram_read"] + L["dram_write"] for L in launches)
