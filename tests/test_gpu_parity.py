@@ -478,3 +478,22 @@ def test_error_codes():
     assert B.lib().hydro_init(C.byref(p), a.data_ptr(), b.data_ptr(), s.data_ptr(), scb - 1, None, C.byref(out)) == B.HYDRO_ENOMEM
     assert B.lib().hydro_init(C.byref(p), a.data_ptr() + 8, b.data_ptr(), s.data_ptr(), scb, None, C.byref(out)) == B.HYDRO_EINVAL
     assert B.lib().hydro_init(C.byref(p), None, b.data_ptr(), s.data_ptr(), scb, None, C.byref(out)) == B.HYDRO_EINVAL
+
+
+@pytest.mark.parametrize("name", ["cfg5_scaling_small", "cfg4_atmosphere_small", "cfg5_256_wide_box"])
+def test_species_groups_in_one_launch_change_no_bit(name, monkeypatch):
+    """HYDRO_SPECIES_ONE_LAUNCH (include/hydro.h): the y and/or z species sweeps with all species groups in one
+    launch (sibling CTAs share rho and F_rho rows through L2) against one launch per group -- identical states."""
+    import torch
+    from paper_2007_05218_b200.binding import Hydro
+    wl = CASES[name]()
+    U0 = W.initial_state(wl)
+    states = []
+    for mode in ("0", "1", "2", "3"):
+        monkeypatch.setenv("HYDRO_SPECIES_ONE_LAUNCH", mode)      # read once per hydro_init
+        h = Hydro(wl.params)
+        assert h.hydro_query(5) == int(mode)
+        h.upload(U0, 0)
+        h.hydro_step(3)
+        states.append(h.U0.clone())
+    assert all(torch.equal(states[0], s) for s in states[1:])
