@@ -192,6 +192,25 @@ def test_config3_ten_ctu_steps_in_one_call():
     assert np.all(np.abs(t1 - t0) <= 1e-13 * scale)
 
 
+def test_config5_and_config4_ctu_steps_at_full_size():
+    """hydro_ctu_step at the two 19-component BASELINE sizes: config 5 (512^3, 5 steps, 13 boxes per batch of the
+    64) and config 4 (256 x 256 x 512 with gravity and reflecting z walls, 10 steps), against oracle_ctu_step on
+    windows that cover the n-step domain of dependence."""
+    import torch
+    wl, U0, h = full_run(5)
+    del U0
+    dts = h.hydro_ctu_step(5, batch_boxes=13, all_dts=True)
+    worst = check_windows(wl, h, dts, [(78, 206, 334), (460, 460, 460)], size=104, tol=1e-10, stepper=O.ctu_step_fixed_dt)
+    print("config 5, 5 CTU steps: worst window error", worst)
+    del h
+    torch.cuda.empty_cache()
+    wl, U0, h = full_run(4)
+    del U0
+    dts = h.hydro_ctu_step(10, all_dts=True)
+    worst = check_windows(wl, h, dts, [(40, 56, 180), (80, 16, None)], size=160, tol=1e-10, stepper=O.ctu_step_fixed_dt)
+    print("config 4, 10 CTU steps: worst window error", worst)
+
+
 def test_config4_atmosphere_sampled_windows():
     wl, U0, h = full_run(4)
     del U0
