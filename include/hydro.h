@@ -68,8 +68,7 @@ typedef struct {
     double  small_dens, small_pres; /* floors (1e-12, 1e-14 in all workloads)                */
     int32_t flatten;            /* 0: off; 1: PPM shock flattening O10, needs ng >= 4 */
     int32_t evolve_eint;        /* 0: rho*e re-synchronised from rho*E after every stage; 1: evolved rho*e with a
-                                   dual-energy switch, O11; needs a geometry the ring kernels
-                                   accept: even ng, even nbox[0] dividing or a multiple of 128 */
+                                   dual-energy switch, O11 */
 } hydro_params;
 
 typedef struct hydro_ctx *hydro_handle;

@@ -414,8 +414,10 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
         else if (g.flatten) launch_hydro_ring<DIR, FINAL, STAGE, true, false>(h, a, grid, state);
         else if (g.evolve) launch_hydro_ring<DIR, FINAL, STAGE, false, true>(h, a, grid, state);
         else launch_hydro_ring<DIR, FINAL, STAGE, false, false>(h, a, grid, state);
-    } else
-        k_sweep_hydro<DIR, FINAL, STAGE, BS><<<grid, BS, 0, h->stream>>>(g, a);
+    } else if (g.evolve)
+        k_sweep_hydro<DIR, FINAL, STAGE, BS, true><<<grid, BS, 0, h->stream>>>(g, a);
+    else
+        k_sweep_hydro<DIR, FINAL, STAGE, BS, false><<<grid, BS, 0, h->stream>>>(g, a);
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
     if (rc) return rc;
     const int ngroups = g.nspec > 0 ? (g.nspec + h->ns_max - 1) / h->ns_max : 0;
@@ -451,7 +453,8 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
         tm.a = h->maps[state][DIR - 1][1];
         tm.b = h->maps[state][DIR - 1][1];
         tm.f = h->fmaps[DIR - 1];
-        if (g.flatten) launch_energy_ring<DIR, FINAL, STAGE, true>(h, a, grid, tm);
+        if (!ring) k_sweep_species<DIR, FINAL, STAGE, 1, BS, FINAL><<<grid, BS, 0, h->stream>>>(g, a);
+        else if (g.flatten) launch_energy_ring<DIR, FINAL, STAGE, true>(h, a, grid, tm);
         else launch_energy_ring<DIR, FINAL, STAGE, false>(h, a, grid, tm);
         if ((rc = check_launch(h, "k_march_species<energy>", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
     }
@@ -836,11 +839,6 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
             std::string why2;
             if (!make_ring_map(&h->fmaps[dir - 1], FL, g, dir, 1, why2, 1, g.cstride)) h->use_ring = false;
         }
-    }
-    if (g.evolve && !h->use_ring) {   // O11 lives in the ring kernels only (even ng, even box width tiling the CTA)
-        delete h;
-        return fail(nullptr, HYDRO_EINVAL, "evolve_eint = 1 needs a geometry the TMA-ring kernels accept "
-                                           "(even ng, even nbox[0] that divides or is a multiple of 128)");
     }
     // a face shared with another shard (HYDRO_BC_EXTERNAL): its ghosts come from hydro_unpack_halo; only the
     // one-launch ghost fill knows how to leave them alone, and hydro_step (no exchange between its stages) is refused

@@ -59,7 +59,7 @@ __device__ __forceinline__ bool pencil(const Geom& g, int seglen, int& i, int& t
 // ------------------------------------------------------------------------------------
 // hydro variables: (rho, u, v, w, p) reconstruction, HLLC, flux difference
 // ------------------------------------------------------------------------------------
-template <int DIR, bool FINAL, int STAGE, int BS>
+template <int DIR, bool FINAL, int STAGE, int BS, bool EVOLVE = false>
 __global__ void __launch_bounds__(BS)
 k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
 {
@@ -83,6 +83,7 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
     double a1[5], a2[5], s1[5], e1[5], aR1[5], Fp[5];
 #pragma unroll
     for (int v = 0; v < 5; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = 0.0; }
+    double ufp = 0.0;                                  // O11: face velocity of the previous face
 
     for (int n = m0 - 3; n <= m1 + 2; ++n) {
         // load zone n, convert to primitives (O2)
@@ -108,12 +109,18 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
             a2[v] = a1[v]; a1[v] = q[v]; s1[v] = sn; e1[v] = en; aR1[v] = aR;
         }
         if (n < m0 + 2) continue;                      // warp-uniform: window still filling
-        double F[5];
-        hllc<DIR>(g, qL, qR, F);                       // face between zones n-3 and n-2
+        double F[5], uf;
+        hllc<DIR>(g, qL, qR, F, uf);                   // face between zones n-3 and n-2
         Fb[(long long)(n - 2) * fmstride] = F[0];
         if (n >= m0 + 3) {
             const int z = n - 3;                       // zone whose two faces are now known
             double* Lz = Lb + z * lmstride;
+            // O11: div(u_face) so far + this direction's part (accumulator slot nflux + 1)
+            double dsum = 0.0;
+            if (EVOLVE) {
+                dsum = Lz[(long long)(g.nflux + 1) * g.lcstride] + (uf - ufp) * dinv;
+                Lz[(long long)(g.nflux + 1) * g.lcstride] = dsum;
+            }
             if (!FINAL) {
 #pragma unroll
                 for (int c = 0; c < 5; ++c) Lz[c * g.lcstride] = Lz[c * g.lcstride] - (F[c] - Fp[c]) * dinv;
@@ -141,12 +148,23 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
                 }
                 const double K = ddiv(HALF * (un[1] * un[1] + un[2] * un[2] + un[3] * un[3]), un[0]);
                 double re = un[4] - K;
-                if (re < g.floor_rhoe) re = g.floor_rhoe;
-                a.Uout[zo + 5 * g.cstride] = re;
+                if (EVOLVE) {      // rho*e is written by the energy launch; leave rho*E - K (slot nflux + 2) for its switch
+                    double eE = re;
+                    if (fabs(re - 1.0e-4 * un[4]) <= 1e-12 * fabs(un[4])) {
+                        // within rounding of the switch threshold: K exactly as the definition forms it (march_ring.cuh)
+                        const double m2 = __dadd_rn(__dadd_rn(__dmul_rn(un[1], un[1]), __dmul_rn(un[2], un[2])), __dmul_rn(un[3], un[3]));
+                        eE = __dsub_rn(un[4], __ddiv_rn(__dmul_rn(HALF, m2), un[0]));
+                    }
+                    Lz[(long long)(g.nflux + 2) * g.lcstride] = eE;
+                } else {
+                    if (re < g.floor_rhoe) re = g.floor_rhoe;
+                    a.Uout[zo + 5 * g.cstride] = re;
+                }
             }
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c) Fp[c] = F[c];
+        ufp = uf;
     }
 }
 
@@ -154,7 +172,9 @@ k_sweep_hydro(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs 
 // passive species: X_k reconstruction, upwinding with the face mass flux (S7)
 // NS species per thread (a1.sbase .. sbase+NS-1)
 // ------------------------------------------------------------------------------------
-template <int DIR, bool FINAL, int STAGE, int NS, int BS>
+// ENERGY (NS = 1, launched with sbase = -1 and lacc_shift = nflux - 4): the one "species" is e = rho*e / rho of O11;
+// its FINAL update adds -p div(u_face) and ends with the dual-energy switch (as k_march_species<ENERGY>).
+template <int DIR, bool FINAL, int STAGE, int NS, int BS, bool ENERGY = false>
 __global__ void __launch_bounds__(BS)
 k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArgs a)
 {
@@ -167,7 +187,7 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
     const long long l0 = ((long long)k * g.nb[1] + j) * g.nb[0] + i;
     const double* Ub = a.Us + (long long)b * g.bstride + z0;
     const double* Xb = Ub + (long long)(6 + a.sbase) * g.cstride;
-    double* Lb = a.Lacc + (long long)b * g.lbstride + l0 + (long long)(5 + a.sbase) * g.lcstride;
+    double* Lb = a.Lacc + (long long)b * g.lbstride + l0 + (long long)(5 + a.sbase + a.lacc_shift) * g.lcstride;
     const long long fmstride = (DIR == 1) ? g.nb[0] : (long long)g.nb[0] * g.nb[1];
     const double* Fb = a.Frho + (long long)b * g.fbstride + ((DIR == 1) ? (long long)k * (g.nb[1] + 1) * g.nb[0] + i
                                                                          : (long long)j * g.nb[0] + i);
@@ -199,7 +219,7 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
             a2[v] = a1[v]; a1[v] = X; s1[v] = sn; e1[v] = en; aR1[v] = aR;
             if (upd) {
                 double* Lz = Lb + z * lmstride + v * g.lcstride;
-                const double L = *Lz - (Fs - Fp[v]) * dinv;
+                double L = *Lz - (Fs - Fp[v]) * dinv;
                 if (!FINAL) {
                     *Lz = L;
                 } else {
@@ -207,7 +227,14 @@ k_sweep_species(const __grid_constant__ Geom g, const __grid_constant__ SweepArg
                                          (long long)(6 + a.sbase + v) * g.cstride;
                     const double us = a.Us[zo];
                     const double ub = (STAGE == 1) ? a.Ubase[zo] : 0.0;
-                    a.Uout[zo] = rk_combine<STAGE>(us, ub, dt, L);
+                    if (ENERGY) L = L - dmax(g.gm1 * us, g.small_pres) * Lz[g.lcstride];      // - p_c * div(u_face)
+                    double un = rk_combine<STAGE>(us, ub, dt, L);
+                    if (ENERGY) {                      // dual-energy switch on the new state, then the floor (G5)
+                        const double eE = Lz[2 * g.lcstride], rEn = a.Uout[zo - g.cstride];
+                        un = (eE > 1.0e-4 * rEn) ? eE : un;
+                        if (un < g.floor_rhoe) un = g.floor_rhoe;
+                    }
+                    a.Uout[zo] = un;
                 }
             }
             Fp[v] = Fs;

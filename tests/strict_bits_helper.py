@@ -23,11 +23,7 @@ for name, make in CASES:
     for opts in ({}, {"flatten": 1}, {"flatten": 1, "evolve_eint": 1}):
         wl = make()
         wl.params.update(opts)
-        try:
-            h = Hydro(wl.params)
-        except Exception:
-            assert opts.get("evolve_eint"), (name, opts)       # only O11 may refuse a geometry (no ring kernels)
-            continue
+        h = Hydro(wl.params)
         U0 = W.initial_state(wl)
         h.upload(U0, 0)
         p = O.make_params(wl.params)

@@ -259,13 +259,35 @@ def test_evolve_with_gravity_and_reflecting_walls_matches_oracle():
     assert np.all(e <= 1e-11), e
 
 
-def test_evolve_rejected_where_the_ring_kernels_cannot_run():
-    from paper_2007_05218_b200 import binding as B
-    wl = CASES["cfg3_one_species_odd_box"]()
-    wl.params["evolve_eint"] = 1
-    with pytest.raises(B.HydroError) as ei:
-        hydro(wl)
-    assert ei.value.code == B.HYDRO_EINVAL
+@pytest.mark.parametrize("ndom,nbox,ng,flatten", [((54, 30, 14), (27, 15, 7), 4, 0), ((32, 32, 32), (16, 16, 16), 5, 1),
+                                                  ((40, 24, 24), (20, 12, 12), 4, 1)])
+def test_evolve_on_geometries_the_ring_kernels_cannot_take(ndom, nbox, ng, flatten):
+    """O11 in the plain-load sweeps (odd box widths, odd ng): the cold-flow recipe of cold_flow() on such boxes."""
+    wl = W.config(3, ndom=ndom, nbox=nbox, nspec=2)
+    wl.params.update(evolve_eint=1, flatten=flatten, ng=ng)
+    G0 = W.gather_valid(wl, W.initial_state(wl))
+    rho = G0[W.RHO]
+    vel = G0[1:4] / rho * 200.0 + np.array([300.0, -150.0, 80.0])[:, None, None, None]
+    G0[1:4] = rho * vel
+    G0[W.EINT] = 0.05 * (1.0 + 0.2 * np.sin(np.arange(ndom[0]) * 2 * np.pi / ndom[0]))[None, None, :]
+    G0[W.EDEN] = G0[W.EINT] + 0.5 * rho * (vel ** 2).sum(axis=0)
+    U0 = W.scatter_valid(wl, G0, ghost_value=np.nan)
+    p = O.make_params(wl.params)
+    h = hydro(wl)
+    assert h.hydro_query(0) == 0                                  # plain-load sweeps
+    h.upload(U0, 0)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.step_explicit()
+    assert abs(dt_g - dt_o) <= 1e-14 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-11), e
+    for s in range(2):
+        dt_o = O.step(p, Uo, Uo1)
+    dt_g = h.hydro_step(2)
+    assert abs(dt_g - dt_o) <= 1e-12 * dt_o
+    e = rel_err(wl, h.download(0).reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-10), e
 
 
 def test_totals_match_oracle_on_same_state():
