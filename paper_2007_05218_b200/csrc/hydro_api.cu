@@ -100,6 +100,7 @@ struct hydro_ctx {
     bool use_xmarch;           // x sweep by the marching kernels of march_x.cuh (else k_sweep_x)
     CUtensorMap xmaps[2][6];   // [state][components per box]: {4 zones, 128 rows} views for the x hydro marching kernel
     CUtensorMap xsmaps[2][6];  // the same with XS_ROWS rows per box, for the x species marching kernels
+    CUtensorMap fxmap;         // {4 columns, XS_ROWS rows} view of the face mass-flux array in its x layout (rows of nb0 + 4)
     std::string err;
     // optional per-launch timing (hydro_profile): event pairs from a pool created by hydro_profile(1);
     // nothing is allocated while launches are recorded (when the pool is used up, recording stops)
@@ -249,6 +250,31 @@ bool make_xmarch_map(CUtensorMap *out, double *U, const Geom &g, int nc, int row
     CUresult r = ((encode_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, U, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                                  CU_TENSOR_MAP_SWIZZLE_NONE, HYDRO_XM_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled failed (" + std::to_string((int)r) + ")"; return false; }
+    return true;
+}
+
+// TMA view of the face mass-flux array in the layout of the x marching kernels: rows of nb0 + 4 columns,
+// [box][k][j][column]; box = XC columns x RJ x RK rows.
+bool make_fx_map(CUtensorMap *out, double *FX, const Geom &g, int rows, std::string &why)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+        why = "cuTensorMapEncodeTiled is not available from the driver";
+        return false;
+    }
+    const int RJ = g.nb[1] < rows ? g.nb[1] : rows, RK = rows / RJ;
+    const cuuint64_t pitch = (cuuint64_t)(g.nb[0] + 4);
+    cuuint64_t dims[4] = {pitch, (cuuint64_t)g.nb[1], (cuuint64_t)g.nb[2], (cuuint64_t)g.nboxes};
+    cuuint64_t strides[3] = {pitch * 8, pitch * g.nb[1] * 8, (cuuint64_t)g.fbstride * 8};
+    cuuint32_t box[4] = {(cuuint32_t)XC, (cuuint32_t)RJ, (cuuint32_t)RK, 1u};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = ((encode_fn)fn)(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, FX, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { why = "cuTensorMapEncodeTiled (FX) failed (" + std::to_string((int)r) + ")"; return false; }
     return true;
 }
 
@@ -464,7 +490,7 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
 template <int N>
 void launch_xmarch_species_n(hydro_handle h, const XArgs &xa, dim3 grid, const XMaps &tm)
 {
-    const size_t sm = (size_t)XM_D * (1 + N) * XS_ROWS * XC * 8 + XM_D * 8;
+    const size_t sm = (size_t)XM_D * (2 + N) * XS_ROWS * XC * 8 + (size_t)2 * XS_ROWS * XC * 8 + XM_D * 8;
 #if HYDRO_XS_MODE
     auto kern = k_xmarch_species<1, N, XS_ROWS, XM_D>;
     const int threads = XS_ROWS * N;
@@ -510,6 +536,7 @@ int xmarch_stage(hydro_handle h, int state, double *Lacc, double *FX)
             xa.sbase = s0;
             tm.a = h->xsmaps[state][1];
             tm.b = h->xsmaps[state][ns];
+            tm.fx = h->fxmap;
             prof_begin(h);
             switch (ns) {
                 case 1: launch_xmarch_species_n<1>(h, xa, sgrid, tm); break;
@@ -828,6 +855,10 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
                 if (!make_xmarch_map(&h->xmaps[st][nc], h->U[st], g, nc, XBS, why2)) h->use_xmarch = false;
                 if (!make_xmarch_map(&h->xsmaps[st][nc], h->U[st], g, nc, XS_ROWS, why2)) h->use_xmarch = false;
             }
+        if (h->use_xmarch) {
+            std::string why2;
+            if (!make_fx_map(&h->fxmap, (double *)(h->scratch + cv.frho), g, XS_ROWS, why2)) h->use_xmarch = false;
+        }
     }
     cudaError_t e = cudaSuccess;
     if (g.flatten) {   // coefficient array = 1 (no flattening) outside the zones k_flatten writes

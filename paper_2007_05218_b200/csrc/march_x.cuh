@@ -46,7 +46,16 @@ struct XArgs {
 
 struct XMaps {
     CUtensorMap a, b;      // {XC, RJ, RK, NCa, 1} and {XC, RJ, RK, NCb, 1} boxes of the stage state
+    CUtensorMap fx;        // {XC, RJ, RK, 1} boxes of the face mass-flux array FX (species kernels)
 };
+
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
 
 // rows of the CTA: RJ consecutive j times RK consecutive k of one box
 struct XRows {
@@ -183,17 +192,20 @@ k_xmarch_hydro(const __grid_constant__ Geom g, const __grid_constant__ XArgs a, 
 // NS species, sbase + set*NS .. of every row, so that the rows of rho are shared by SETS thread sets: more
 // threads per row stream in flight (the L2 holds the 128-byte lines of which a step consumes 32 bytes; their
 // number, not the thread count, is what has to stay small -- profiles/r02_xmarch.md).
-// Ring rows: rho (map a, 1 component) + rho*X_k, k = sbase .. sbase + NS*SETS - 1 (map b).  F_rho of the four
-// faces of a ring step is one 256-bit load, issued one step ahead.
+// Ring rows: rho (map a, 1 component), F_rho,x of the four faces of the step (map fx), rho*X_k, k = sbase ..
+// sbase + NS*SETS - 1 (map b): no thread loads anything from global memory.  The four reciprocal densities of a
+// row and step are formed once (by different thread sets) and shared through shared memory.
 template <int NS, int SETS, int ROWS, int D>
 __global__ void __launch_bounds__(ROWS * SETS, XM_MINB_S)
 k_xmarch_species(const __grid_constant__ Geom g, const __grid_constant__ XArgs a, const __grid_constant__ XMaps tm)
 {
-    constexpr int NROW = 1 + NS * SETS;
+    // ring rows: rho, F_rho,x of the step's four faces (map fx over the FX array), then the NS * SETS species
+    constexpr int NROW = 2 + NS * SETS;
     constexpr int SLOT = NROW * ROWS * XC;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * SLOT * 8);
+    double* rinvs = ring + (size_t)D * SLOT;                     // 1 / rho of the step's zones, two buffers by step parity
+    uint64_t* full = reinterpret_cast<uint64_t*>(rinvs + 2 * ROWS * XC);
 
     const int tid = threadIdx.x;
     const int set = tid / ROWS, row = tid - set * ROWS;
@@ -207,12 +219,14 @@ k_xmarch_species(const __grid_constant__ Geom g, const __grid_constant__ XArgs a
         mbar_expect_tx(bar, (uint32_t)(SLOT * 8));
         const int c0 = XC * (it - 1) + g.ng;
         tma_load_5d(slot, &tm.a, bar, c0, r.j0 + g.ng, r.k0 + g.ng, 0, r.b);
-        tma_load_5d(slot + ROWS * XC, &tm.b, bar, c0, r.j0 + g.ng, r.k0 + g.ng, 6 + sbase, r.b);
+        tma_load_4d(slot + ROWS * XC, &tm.fx, bar, XC * (it - 1), r.j0, r.k0, r.b);     // columns < 0 (step 0): zero fill
+        tma_load_5d(slot + 2 * ROWS * XC, &tm.b, bar, c0, r.j0 + g.ng, r.k0 + g.ng, 6 + sbase, r.b);
     };
 
     if (tid == 0) {
         tma_prefetch_desc(&tm.a);
         tma_prefetch_desc(&tm.b);
+        tma_prefetch_desc(&tm.fx);
         for (int s = 0; s < D; ++s) mbar_init(&full[s], 1);
         mbar_fence_init();
     }
@@ -220,31 +234,27 @@ k_xmarch_species(const __grid_constant__ Geom g, const __grid_constant__ XArgs a
     if (tid == 0)
         for (int it = 0; it < D && it < nsteps; ++it) issue(it);
 
-    // inactive rows (k beyond the box in the last row tile) read row 0 of the face array and store nothing
-    const long long rowid = r.active ? (long long)r.k * g.nb[1] + r.j : 0;
+    const long long rowid = (long long)r.k * g.nb[1] + r.j;
     double* Lrow = a.Lacc + (long long)r.b * g.lbstride + (long long)(5 + sbase + set * NS) * g.lcstride + rowid * g.nb[0] - 2 * XC;
-    const double* Frow = a.FX + (long long)r.b * g.fbstride + rowid * (g.nb[0] + 4) - XC;
     const double dinv = g.dxinv[0];
 
     double a1[NS], a2[NS], s1[NS], e1[NS], aR1[NS], Fp[NS], carry[NS];
 #pragma unroll
     for (int v = 0; v < NS; ++v) { a1[v] = a2[v] = s1[v] = e1[v] = aR1[v] = Fp[v] = carry[v] = 0.0; }
-    double fn[XC] = {0.0, 0.0, 0.0, 0.0};      // F_rho of the faces of the next step
-    if (nsteps > 1) ld4(Frow + XC, fn[0], fn[1], fn[2], fn[3]);
 
     for (int it = 0; it < nsteps; ++it) {
-        double fr[XC];
-#pragma unroll
-        for (int q = 0; q < XC; ++q) fr[q] = fn[q];
-        if (it >= 1 && it + 1 < nsteps) ld4(Frow + XC * (it + 1), fn[0], fn[1], fn[2], fn[3]);
         const double* sl = ring + (size_t)(it % D) * SLOT + row * XC;
-        const double* sx = sl + (1 + set * NS) * ROWS * XC;
+        const double* sx = sl + (2 + set * NS) * ROWS * XC;
+        double* rs = rinvs + (it & 1) * ROWS * XC + row;          // [zone of the step][row]: conflict-free both ways
         mbar_wait(&full[it % D], (uint32_t)((it / D) & 1));
+        // the reciprocal densities of the step's zones are formed once per row: thread set s takes zone s (, s + SETS ..)
+        for (int q = set; q < XC; q += SETS) rs[q * ROWS] = drcp(dmax(sl[q], g.small_dens));
+        __syncthreads();
         double acc[NS][XC];
 #pragma unroll
         for (int q = 0; q < XC; ++q) {
-            const double rinv = drcp(dmax(sl[q], g.small_dens));
-            const double Frho = (it >= 1) ? fr[q] : 0.0;
+            const double rinv = rs[q * ROWS];
+            const double Frho = sl[ROWS * XC + q];
 #pragma unroll
             for (int v = 0; v < NS; ++v) {
                 const double X = sx[v * ROWS * XC + q] * rinv;
