@@ -69,7 +69,9 @@ typedef struct {
                                    with a dual-energy switch, O11 */
 } oracle_params;
 
-enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2 };
+enum { BC_PERIODIC = 0, BC_OUTFLOW = 1, BC_REFLECT = 2, BC_EXTERNAL = 3 };
+/* BC_EXTERNAL: the ghost zones across the face are somebody else's to fill (another shard, or the coarser level:
+ * oracle_fill_from_coarse); oracle_fill_ghosts leaves them alone. */
 
 static double dmin(double a, double b) { return a < b ? a : b; }
 static double dmax(double a, double b) { return a > b ? a : b; }
@@ -101,7 +103,7 @@ static int make_geom(const oracle_params *p, geom_t *g)
         if (p->ndom[d] <= 0 || p->nbox[d] <= 0) return -1;
         if (p->ndom[d] % p->nbox[d] != 0) return -1;
         if ((p->bc_lo[d] == BC_PERIODIC) != (p->bc_hi[d] == BC_PERIODIC)) return -1;
-        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 2 || p->bc_hi[d] < 0 || p->bc_hi[d] > 2) return -1;
+        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 3 || p->bc_hi[d] < 0 || p->bc_hi[d] > 3) return -1;
         g->nb[d] = p->nbox[d];
         g->nt[d] = p->nbox[d] + 2 * p->ng;
         g->NB[d] = p->ndom[d] / p->nbox[d];
@@ -137,6 +139,7 @@ static int map_global(const oracle_params *p, int d, int gidx, int *sgn)
     int bc = gidx < 0 ? p->bc_lo[d] : p->bc_hi[d];
     if (bc == BC_PERIODIC) return ((gidx % n) + n) % n;
     if (bc == BC_OUTFLOW) return gidx < 0 ? 0 : n - 1;
+    if (bc == BC_EXTERNAL) return -1;
     /* reflect */
     *sgn = -1;
     return gidx < 0 ? -1 - gidx : 2 * n - 1 - gidx;
@@ -161,6 +164,7 @@ int oracle_fill_ghosts(const oracle_params *p, double *U)
             int gx = map_global(p, 0, bi * g.nb[0] + il - ng, &sg[0]);
             int gy = map_global(p, 1, bj * g.nb[1] + jl - ng, &sg[1]);
             int gz = map_global(p, 2, bk * g.nb[2] + kl - ng, &sg[2]);
+            if (gx < 0 || gy < 0 || gz < 0) continue;      /* across an external face: not ours to fill */
             size_t sb = ((size_t)(gz / g.nb[2]) * g.NB[1] + gy / g.nb[1]) * g.NB[0] + gx / g.nb[0];
             size_t sz = zidx(&g, gx % g.nb[0] + ng, gy % g.nb[1] + ng, gz % g.nb[2] + ng);
             size_t dz = zidx(&g, il, jl, kl);
@@ -930,5 +934,94 @@ int oracle_ctu_step(const oracle_params *p, double *U0, double *U1, double *dt_o
     if (rc) return rc;
     if ((rc = oracle_ctu_step_fixed_dt(p, U0, U1, dt))) return rc;
     if (dt_out) *dt_out = dt;
+    return 0;
+}
+
+/* =====================================================================================================
+ * O13 (second half; "a MultiFab ... at a given level of mesh refinement",
+ * PAPER.md:149 refinement by factors of 4): two-level ghost fill.  The FINE level is a rectangular patch of the
+ * coarse domain, refined by `ratio` (2 or 4) in every direction and tiled by its own boxes; its faces that lie
+ * inside the coarse domain are BC_EXTERNAL.  Every fine ghost zone across such a face takes its NVAR components
+ * from the coarse level by conservative linear interpolation.  The paper prints none of this; readings:
+ *  A1  the fine global index gf (negative or >= ndom_f across a face) belongs to the coarse zone
+ *      gc = lo + floor(gf / ratio), child position r = gf - ratio*floor(gf / ratio) in 0 .. ratio-1;
+ *  A2  value = Uc + sx*xi_x + sy*xi_y + sz*xi_z (left to right), xi = (r + 0.5)/ratio - 0.5, per component;
+ *  A3  slopes per coarse zone and dimension = the limited slope of O3 (CW84 1.7-1.8) of the coarse zone averages
+ *      gc-1, gc, gc+1: monotone, exact for linear data, and the children of a zone average to its value;
+ *  A4  coarse zones outside the coarse domain are the coarse level's own ghost zones (its boundary conditions
+ *      apply; they must be filled first), looked up in the box nearest to them;
+ *  A5  a fine ghost zone is filled here iff its index is across an EXTERNAL face in at least one dimension;
+ *      the other fine ghost zones (fine-fine neighbours, physical boundaries of the patch) are O1's.
+ * Pins (tests/test_oracle_amr.py): linear data reproduced bit for bit (dyadic coefficients), constants, child
+ * means, a local extremum interpolates flat, every EXTERNAL-side ghost zone and no other zone is written, ratio 4.
+ * ===================================================================================================== */
+static int floor_div_i(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+
+/* value of component c at coarse GLOBAL zone gidx[3] (may lie up to ng zones outside the domain) */
+static int coarse_at(const geom_t *gc, const double *Uc, int c, const int *gidx, double *out)
+{
+    size_t b = 0;
+    int l[3];
+    int bd[3];
+    for (int d = 0; d < 3; ++d) {
+        bd[d] = floor_div_i(gidx[d], gc->nb[d]);
+        if (bd[d] < 0) bd[d] = 0;
+        if (bd[d] > gc->NB[d] - 1) bd[d] = gc->NB[d] - 1;
+        l[d] = gidx[d] - bd[d] * gc->nb[d] + gc->ng;
+        if (l[d] < 0 || l[d] >= gc->nt[d]) return -1;
+    }
+    b = ((size_t)bd[2] * gc->NB[1] + bd[1]) * gc->NB[0] + bd[0];
+    *out = Uc[b * gc->box_stride + (size_t)c * gc->comp_stride + zidx(gc, l[0], l[1], l[2])];
+    return 0;
+}
+
+int oracle_fill_from_coarse(const oracle_params *pf, double *Uf, const oracle_params *pc, const double *Uc,
+                            const int32_t *lo, int ratio)
+{
+    geom_t gf, gc;
+    if (make_geom(pf, &gf) || make_geom(pc, &gc) || !Uf || !Uc || !lo) return -1;
+    if ((ratio != 2 && ratio != 4) || pf->nspec != pc->nspec) return -1;
+    for (int d = 0; d < 3; ++d) {
+        if (pf->ndom[d] % ratio) return -1;
+        if (lo[d] < 0 || lo[d] + pf->ndom[d] / ratio > pc->ndom[d]) return -1;
+    }
+    const int ng = gf.ng;
+    for (int bk = 0; bk < gf.NB[2]; ++bk)
+    for (int bj = 0; bj < gf.NB[1]; ++bj)
+    for (int bi = 0; bi < gf.NB[0]; ++bi) {
+        size_t b = ((size_t)bk * gf.NB[1] + bj) * gf.NB[0] + bi;
+        const int bb[3] = { bi, bj, bk };
+        for (int kl = 0; kl < gf.nt[2]; ++kl)
+        for (int jl = 0; jl < gf.nt[1]; ++jl)
+        for (int il = 0; il < gf.nt[0]; ++il) {
+            const int ll[3] = { il, jl, kl };
+            int g[3], cz[3], ext = 0;
+            double xi[3];
+            for (int d = 0; d < 3; ++d) {
+                g[d] = bb[d] * gf.nb[d] + ll[d] - ng;
+                if ((g[d] < 0 && pf->bc_lo[d] == BC_EXTERNAL) || (g[d] >= pf->ndom[d] && pf->bc_hi[d] == BC_EXTERNAL)) ext = 1;
+                int q = floor_div_i(g[d], ratio);
+                cz[d] = lo[d] + q;
+                xi[d] = ((double)(g[d] - ratio * q) + 0.5) / (double)ratio - 0.5;
+            }
+            if (!ext) continue;
+            size_t dz = b * gf.box_stride + zidx(&gf, il, jl, kl);
+            for (int c = 0; c < gf.nvar; ++c) {
+                double u0;
+                if (coarse_at(&gc, Uc, c, cz, &u0)) return -1;
+                double val = u0;
+                for (int d = 0; d < 3; ++d) {
+                    int cm[3] = { cz[0], cz[1], cz[2] }, cp[3] = { cz[0], cz[1], cz[2] };
+                    cm[d] -= 1; cp[d] += 1;
+                    double um, up;
+                    if (coarse_at(&gc, Uc, c, cm, &um) || coarse_at(&gc, Uc, c, cp, &up)) return -1;
+                    double dp = up - u0, dm = u0 - um, dc = HALF * (up - um), sl = 0.0;
+                    if (dp * dm > 0.0) sl = copysign(dmin(fabs(dc), dmin(2.0 * fabs(dp), 2.0 * fabs(dm))), dc);
+                    val = val + sl * xi[d];
+                }
+                Uf[dz + (size_t)c * gf.comp_stride] = val;
+            }
+        }
+    }
     return 0;
 }

@@ -66,6 +66,7 @@ def lib():
         L.oracle_ctu_step_fixed_dt.argtypes = [pp, dp, dp, C.c_double]
         L.oracle_ctu_trace.restype = None
         L.oracle_ctu_trace.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_double, dp, dp, dp, dp, dp]
+        L.oracle_fill_from_coarse.argtypes = [pp, dp, pp, dp, C.POINTER(C.c_int32), C.c_int]
         L.oracle_max_threads.restype = C.c_int
         L.oracle_set_threads.restype = None
         L.oracle_set_threads.argtypes = [C.c_int]
@@ -179,3 +180,9 @@ def ctu_trace(d, gamma, small_dens, small_pres, dtdx, a, aL, aR):
     qm, qp = np.zeros_like(a), np.zeros_like(a)
     lib().oracle_ctu_trace(d, gamma, small_dens, small_pres, a.size - 5, dtdx, _ptr(a), _ptr(aL), _ptr(aR), _ptr(qm), _ptr(qp))
     return qm, qp
+
+
+def fill_from_coarse(pf, Uf, pc, Uc, lo, ratio):
+    """O13: fine ghost zones across EXTERNAL faces from the coarse level (conservative linear interpolation)."""
+    lo3 = (C.c_int32 * 3)(*[int(x) for x in lo])
+    _check(lib().oracle_fill_from_coarse(C.byref(pf), _ptr(Uf), C.byref(pc), _ptr(Uc), lo3, int(ratio)), "fill_from_coarse")
