@@ -166,6 +166,21 @@ size_t hydro_halo_bytes(const hydro_params *p, int dim);
 int hydro_pack_halo(hydro_handle h, int which, int dim, int side, void *buf_dev);
 int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *buf_dev);
 
+/* O13 two-level ghost fill (second half; PAPER.md:35 a MultiFab lives
+ * "at a given level of mesh refinement", PAPER.md:149 refinement by factors of 4).  `fine` is the handle of a
+ * rectangular patch of `coarse`'s domain refined by ratio (2 or 4) in every direction: fine ndom = ratio * (patch
+ * extent in coarse zones), prob_lo / prob_hi = the patch, its own boxes and ghost zones; the faces of the patch that
+ * lie inside the coarse domain are HYDRO_BC_EXTERNAL, the others carry the physical boundary type.  The call fills
+ * every ghost zone of fine state `which_fine` whose index lies across an EXTERNAL face in at least one dimension
+ * from coarse state `which_coarse` (ghosts filled!) by conservative linear interpolation: value = Uc + sum_d
+ * slope_d * xi_d, slope_d = the limited slope of O3 of the coarse zone averages, xi_d = (child + 0.5)/ratio - 0.5
+ * (children average to their parent, linear data are reproduced exactly, no new extrema).  The other fine ghost
+ * zones are hydro_fill_ghosts's.  lo_coarse[3] (HOST): coarse zone of the patch's first fine zone.  Both handles on
+ * one device; the coarse level needs (ng_fine + ratio - 1)/ratio + 1 <= ng_coarse ghost zones.  Asynchronous on the
+ * fine handle's stream (ordered after the coarse handle's stream). */
+int hydro_fill_from_coarse(hydro_handle fine, int which_fine, hydro_handle coarse, int which_coarse,
+                           const int32_t *lo_coarse, int ratio);
+
 /* Which internal paths this handle uses (for bench accounting; they change no result):
  * what = 0: TMA-ring marching kernels (1) or the plain-load fallback (0);
  *        1: hydro_step fills ghosts in two parts (x images written by the z sweeps + ghost-row

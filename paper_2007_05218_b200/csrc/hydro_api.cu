@@ -19,6 +19,7 @@
 #include "march_ring.cuh"
 #include "march_x.cuh"
 #include "ctu.cuh"
+#include "amr_fill.cuh"
 
 using namespace hydro;
 
@@ -1019,6 +1020,42 @@ int hydro_ctu_step(hydro_handle h, void *ctu_scratch_dev, size_t ctu_scratch_byt
         if (e != cudaSuccess && rc == HYDRO_OK) rc = fail(h, HYDRO_ECUDA, std::string("CTU copy back: ") + cudaGetErrorString(e));
     }
     return rc;
+}
+
+int hydro_fill_from_coarse(hydro_handle fine, int which_fine, hydro_handle coarse, int which_coarse, const int32_t *lo_coarse,
+                           int ratio)
+{
+    if (!fine || !coarse) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    hydro_handle h = fine;
+    if ((which_fine != 0 && which_fine != 1) || (which_coarse != 0 && which_coarse != 1))
+        return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
+    if (!lo_coarse) return fail(h, HYDRO_EINVAL, "null lo_coarse");
+    if (ratio != 2 && ratio != 4) return fail(h, HYDRO_EINVAL, "ratio must be 2 or 4");
+    const Geom &gf = fine->g, &gc = coarse->g;
+    if (fine->device != coarse->device) return fail(h, HYDRO_EINVAL, "the two levels must live on one device");
+    if (gf.nvar != gc.nvar) return fail(h, HYDRO_EINVAL, "the two levels must carry the same components");
+    AmrArgs a;
+    for (int d = 0; d < 3; ++d) {
+        if (gf.ndom[d] % ratio) return fail(h, HYDRO_EINVAL, "the fine patch must cover whole coarse zones");
+        if (lo_coarse[d] < 0 || lo_coarse[d] + gf.ndom[d] / ratio > gc.ndom[d])
+            return fail(h, HYDRO_EINVAL, "the fine patch must lie inside the coarse domain");
+        // the deepest fine ghost zone needs the coarse zone (ng_f + ratio - 1)/ratio outside the patch, and its slope one more
+        if ((gf.ng + ratio - 1) / ratio + 1 > gc.ng) return fail(h, HYDRO_EINVAL, "coarse level has too few ghost zones for this ratio");
+        a.lo[d] = lo_coarse[d];
+    }
+    if (gf.nt[2] > 65535 || gf.nboxes > 65535) return fail(h, HYDRO_EINVAL, "fine level grid too large for the coarse-fine fill");
+    a.Uf = fine->U[which_fine]; a.Uc = coarse->U[which_coarse]; a.ratio = ratio;
+    DeviceGuard guard(h->device);
+    if (coarse->stream != fine->stream) {      // order after the coarse level's work (its ghost fill)
+        cudaEvent_t ev;
+        if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) return fail(h, HYDRO_ECUDA, "event creation failed");
+        cudaEventRecord(ev, coarse->stream);
+        cudaStreamWaitEvent(fine->stream, ev, 0);
+        cudaEventDestroy(ev);
+    }
+    prof_begin(h);
+    k_fill_from_coarse<<<dim3((gf.nt[0] * gf.nt[1] + 255) / 256, gf.nt[2], gf.nboxes), 256, 0, h->stream>>>(gf, gc, a);
+    return check_launch(h, "k_fill_from_coarse", K_GHOST);
 }
 
 int hydro_query(hydro_handle h, int what)
