@@ -181,6 +181,13 @@ int hydro_unpack_halo(hydro_handle h, int which, int dim, int side, const void *
 int hydro_fill_from_coarse(hydro_handle fine, int which_fine, hydro_handle coarse, int which_coarse,
                            const int32_t *lo_coarse, int ratio);
 
+/* O13 restriction: every VALID zone of coarse state `which_coarse` that the patch covers becomes the mean of its
+ * ratio^3 fine children (all NVAR components; conservative: the children's volumes add up to the parent's).  Same
+ * patch description and checks as hydro_fill_from_coarse.  Asynchronous on the coarse handle's stream (ordered after
+ * the fine handle's stream). */
+int hydro_average_down(hydro_handle coarse, int which_coarse, hydro_handle fine, int which_fine,
+                       const int32_t *lo_coarse, int ratio);
+
 /* Which internal paths this handle uses (for bench accounting; they change no result):
  * what = 0: TMA-ring marching kernels (1) or the plain-load fallback (0);
  *        1: hydro_step fills ghosts in two parts (x images written by the z sweeps + ghost-row

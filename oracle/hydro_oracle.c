@@ -1025,3 +1025,40 @@ int oracle_fill_from_coarse(const oracle_params *pf, double *Uf, const oracle_pa
     }
     return 0;
 }
+
+/* O13, restriction (reading A6): every coarse VALID zone covered by the patch becomes the mean of its ratio^3 fine
+ * children, summed in the order k, j, i (i innermost) and multiplied by 1/ratio^3 (exact: 1/8 or 1/64), all NVAR
+ * components -- the conservative average-down of an AMR hierarchy (volumes of the children add up to the parent's).
+ * Pins: constants and dyadic linear fields exact, the coarse total over the patch equals the fine total. */
+int oracle_average_down(const oracle_params *pc, double *Uc, const oracle_params *pf, const double *Uf,
+                        const int32_t *lo, int ratio)
+{
+    geom_t gf, gc;
+    if (make_geom(pf, &gf) || make_geom(pc, &gc) || !Uf || !Uc || !lo) return -1;
+    if ((ratio != 2 && ratio != 4) || pf->nspec != pc->nspec) return -1;
+    for (int d = 0; d < 3; ++d) {
+        if (pf->ndom[d] % ratio) return -1;
+        if (lo[d] < 0 || lo[d] + pf->ndom[d] / ratio > pc->ndom[d]) return -1;
+    }
+    const double inv = 1.0 / (double)(ratio * ratio * ratio);
+    for (int K = 0; K < pf->ndom[2] / ratio; ++K)
+    for (int J = 0; J < pf->ndom[1] / ratio; ++J)
+    for (int I = 0; I < pf->ndom[0] / ratio; ++I) {
+        const int G[3] = { lo[0] + I, lo[1] + J, lo[2] + K };
+        size_t cb = ((size_t)(G[2] / gc.nb[2]) * gc.NB[1] + G[1] / gc.nb[1]) * gc.NB[0] + G[0] / gc.nb[0];
+        size_t cz = cb * gc.box_stride + zidx(&gc, G[0] % gc.nb[0] + gc.ng, G[1] % gc.nb[1] + gc.ng, G[2] % gc.nb[2] + gc.ng);
+        for (int c = 0; c < gc.nvar; ++c) {
+            double sum = 0.0;
+            for (int kk = 0; kk < ratio; ++kk)
+            for (int jj = 0; jj < ratio; ++jj)
+            for (int ii = 0; ii < ratio; ++ii) {
+                const int g[3] = { I * ratio + ii, J * ratio + jj, K * ratio + kk };
+                size_t fb = ((size_t)(g[2] / gf.nb[2]) * gf.NB[1] + g[1] / gf.nb[1]) * gf.NB[0] + g[0] / gf.nb[0];
+                sum = sum + Uf[fb * gf.box_stride + (size_t)c * gf.comp_stride +
+                               zidx(&gf, g[0] % gf.nb[0] + gf.ng, g[1] % gf.nb[1] + gf.ng, g[2] % gf.nb[2] + gf.ng)];
+            }
+            Uc[cz + (size_t)c * gc.comp_stride] = sum * inv;
+        }
+    }
+    return 0;
+}

@@ -67,6 +67,7 @@ def lib():
         L.oracle_ctu_trace.restype = None
         L.oracle_ctu_trace.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_int, C.c_double, dp, dp, dp, dp, dp]
         L.oracle_fill_from_coarse.argtypes = [pp, dp, pp, dp, C.POINTER(C.c_int32), C.c_int]
+        L.oracle_average_down.argtypes = [pp, dp, pp, dp, C.POINTER(C.c_int32), C.c_int]
         L.oracle_max_threads.restype = C.c_int
         L.oracle_set_threads.restype = None
         L.oracle_set_threads.argtypes = [C.c_int]
@@ -186,3 +187,9 @@ def fill_from_coarse(pf, Uf, pc, Uc, lo, ratio):
     """O13: fine ghost zones across EXTERNAL faces from the coarse level (conservative linear interpolation)."""
     lo3 = (C.c_int32 * 3)(*[int(x) for x in lo])
     _check(lib().oracle_fill_from_coarse(C.byref(pf), _ptr(Uf), C.byref(pc), _ptr(Uc), lo3, int(ratio)), "fill_from_coarse")
+
+
+def average_down(pc, Uc, pf, Uf, lo, ratio):
+    """O13 restriction: coarse valid zones under the patch <- mean of their fine children."""
+    lo3 = (C.c_int32 * 3)(*[int(x) for x in lo])
+    _check(lib().oracle_average_down(C.byref(pc), _ptr(Uc), C.byref(pf), _ptr(Uf), lo3, int(ratio)), "average_down")

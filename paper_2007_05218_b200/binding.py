@@ -16,7 +16,7 @@ HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3,
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
            "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host",
-           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo", "hydro_ctu_scratch_bytes", "hydro_ctu_step", "hydro_fill_from_coarse"]
+           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo", "hydro_ctu_scratch_bytes", "hydro_ctu_step", "hydro_fill_from_coarse", "hydro_average_down"]
 PROBE_LIB_PATH = os.path.join(HERE, "libhydro_probe_b200.so")
 PROBE_EXPORTS = ["hydro_probe_fp64"]
 
@@ -89,6 +89,7 @@ def lib():
     L.hydro_ctu_scratch_bytes.argtypes = [pp]
     L.hydro_ctu_step.argtypes = [vp, vp, C.c_size_t, C.c_int, dp]
     L.hydro_fill_from_coarse.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int32), C.c_int]
+    L.hydro_average_down.argtypes = [vp, C.c_int, vp, C.c_int, C.POINTER(C.c_int32), C.c_int]
     L.hydro_halo_bytes.restype = C.c_size_t
     L.hydro_halo_bytes.argtypes = [pp, C.c_int]
     L.hydro_pack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
@@ -227,6 +228,11 @@ class Hydro:
         """self = the refined patch; coarse = the Hydro of the coarse level (include/hydro.h, O13)."""
         lo = (C.c_int32 * 3)(*[int(x) for x in lo_coarse])
         self._check(lib().hydro_fill_from_coarse(self.h, which, coarse.h, which_coarse, lo, int(ratio)))
+
+    def hydro_average_down(self, which, fine, which_fine, lo_coarse, ratio):
+        """self = the coarse level; fine = the Hydro of the refined patch (include/hydro.h, O13 restriction)."""
+        lo = (C.c_int32 * 3)(*[int(x) for x in lo_coarse])
+        self._check(lib().hydro_average_down(self.h, which, fine.h, which_fine, lo, int(ratio)))
 
     def hydro_pack_halo(self, which, dim, side, buf):
         """buf: device tensor of hydro_halo_bytes(params, dim) bytes (sharded.py)."""

@@ -78,4 +78,31 @@ k_fill_from_coarse(const __grid_constant__ Geom gf, const __grid_constant__ Geom
     }
 }
 
+// restriction (reading A6): coarse valid zone under the patch <- mean of its ratio^3 children, summed k, j, i (i innermost).
+// One thread per (coarse zone of the patch, component): grid (ceil(zones / 256), nvar).
+__global__ void __launch_bounds__(256)
+k_average_down(const __grid_constant__ Geom gc, const __grid_constant__ Geom gf, double* __restrict__ Uc,
+               const double* __restrict__ Uf, int lo0, int lo1, int lo2, int ratio)
+{
+    const int n0 = gf.ndom[0] / ratio, n1 = gf.ndom[1] / ratio, n2 = gf.ndom[2] / ratio;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n0 * n1 * n2) return;
+    const int I = (int)(t % n0), J = (int)((t / n0) % n1), K = (int)(t / ((long long)n0 * n1));
+    const int c = blockIdx.y;
+    const int G[3] = {lo0 + I, lo1 + J, lo2 + K};
+    const long long cb = ((long long)(G[2] / gc.nb[2]) * gc.NB[1] + G[1] / gc.nb[1]) * gc.NB[0] + G[0] / gc.nb[0];
+    const long long cz = cb * gc.bstride + (long long)c * gc.cstride +
+                         ((long long)(G[2] % gc.nb[2] + gc.ng) * gc.nt[1] + (G[1] % gc.nb[1] + gc.ng)) * gc.nt[0] + (G[0] % gc.nb[0] + gc.ng);
+    double sum = 0.0;
+    for (int kk = 0; kk < ratio; ++kk)
+        for (int jj = 0; jj < ratio; ++jj)
+            for (int ii = 0; ii < ratio; ++ii) {
+                const int g[3] = {I * ratio + ii, J * ratio + jj, K * ratio + kk};
+                const long long fb = ((long long)(g[2] / gf.nb[2]) * gf.NB[1] + g[1] / gf.nb[1]) * gf.NB[0] + g[0] / gf.nb[0];
+                sum = sum + __ldg(Uf + fb * gf.bstride + (long long)c * gf.cstride +
+                                  ((long long)(g[2] % gf.nb[2] + gf.ng) * gf.nt[1] + (g[1] % gf.nb[1] + gf.ng)) * gf.nt[0] + (g[0] % gf.nb[0] + gf.ng));
+            }
+    Uc[cz] = sum * (1.0 / (double)(ratio * ratio * ratio));
+}
+
 }  // namespace hydro

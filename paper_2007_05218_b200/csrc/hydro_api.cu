@@ -1058,6 +1058,37 @@ int hydro_fill_from_coarse(hydro_handle fine, int which_fine, hydro_handle coars
     return check_launch(h, "k_fill_from_coarse", K_GHOST);
 }
 
+int hydro_average_down(hydro_handle coarse, int which_coarse, hydro_handle fine, int which_fine, const int32_t *lo_coarse, int ratio)
+{
+    if (!fine || !coarse) return fail(nullptr, HYDRO_EINVAL, "null handle");
+    hydro_handle h = coarse;
+    if ((which_fine != 0 && which_fine != 1) || (which_coarse != 0 && which_coarse != 1))
+        return fail(h, HYDRO_EINVAL, "which must be 0 or 1");
+    if (!lo_coarse) return fail(h, HYDRO_EINVAL, "null lo_coarse");
+    if (ratio != 2 && ratio != 4) return fail(h, HYDRO_EINVAL, "ratio must be 2 or 4");
+    const Geom &gf = fine->g, &gc = coarse->g;
+    if (fine->device != coarse->device) return fail(h, HYDRO_EINVAL, "the two levels must live on one device");
+    if (gf.nvar != gc.nvar) return fail(h, HYDRO_EINVAL, "the two levels must carry the same components");
+    for (int d = 0; d < 3; ++d) {
+        if (gf.ndom[d] % ratio) return fail(h, HYDRO_EINVAL, "the fine patch must cover whole coarse zones");
+        if (lo_coarse[d] < 0 || lo_coarse[d] + gf.ndom[d] / ratio > gc.ndom[d])
+            return fail(h, HYDRO_EINVAL, "the fine patch must lie inside the coarse domain");
+    }
+    DeviceGuard guard(h->device);
+    if (coarse->stream != fine->stream) {      // order after the fine level's work
+        cudaEvent_t ev;
+        if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) return fail(h, HYDRO_ECUDA, "event creation failed");
+        cudaEventRecord(ev, fine->stream);
+        cudaStreamWaitEvent(coarse->stream, ev, 0);
+        cudaEventDestroy(ev);
+    }
+    const long long zones = (long long)(gf.ndom[0] / ratio) * (gf.ndom[1] / ratio) * (gf.ndom[2] / ratio);
+    prof_begin(h);
+    k_average_down<<<dim3((unsigned)((zones + 255) / 256), gc.nvar), 256, 0, h->stream>>>(gc, gf, coarse->U[which_coarse], fine->U[which_fine],
+                                                                                          lo_coarse[0], lo_coarse[1], lo_coarse[2], ratio);
+    return check_launch(h, "k_average_down", K_GHOST);
+}
+
 int hydro_query(hydro_handle h, int what)
 {
     if (!h) return -1;

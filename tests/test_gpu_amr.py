@@ -98,3 +98,18 @@ def test_one_rk2_step_of_a_refined_patch_inside_a_coarse_level():
     e = rel_err(wf, hf.download(0).reshape(Uf.shape), Uf)
     assert np.all(e <= 1e-12), e
     assert np.abs(W.gather_valid(wf, Uf) - Gf).max() > 1e-4          # the patch did evolve
+
+
+@pytest.mark.parametrize("ratio", [2, 4])
+def test_average_down_bit_for_bit(ratio):
+    wc, wf = levels(ratio=ratio, lo=(4, 2, 6), patch=(8, 4, 6), nbox_c=(8, 16, 8), nspec=2)
+    wf.params["nbox"] = [wf.params["ndom"][0] // 2, wf.params["ndom"][1], wf.params["ndom"][2] // 2]
+    rng = np.random.default_rng(21)
+    nf = wf.params["ndom"]
+    Uf = W.scatter_valid(wf, rng.standard_normal((wf.nvar, nf[2], nf[1], nf[0])), ghost_value=np.nan)
+    Uc = W.scatter_valid(wc, rng.standard_normal((wc.nvar, 16, 16, 16)), ghost_value=np.nan)
+    hc, hf = hydro(wc), hydro(wf)
+    hc.upload(Uc, 1); hf.upload(Uf, 0)
+    hc.hydro_average_down(1, hf, 0, (4, 2, 6), ratio)
+    O.average_down(O.make_params(wc.params), Uc, O.make_params(wf.params), Uf, (4, 2, 6), ratio)
+    assert np.array_equal(hc.download(1), Uc, equal_nan=True)

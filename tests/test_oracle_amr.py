@@ -139,3 +139,36 @@ def test_fill_ghosts_leaves_external_faces_alone_and_rejects_bad_patches():
         O.fill_from_coarse(pf, U, pc, Uc, (4, 4, 4), 3)                      # ratio must be 2 or 4
     with pytest.raises(RuntimeError):
         O.fill_from_coarse(pf, U, pc, Uc, (12, 4, 4), 2)                     # the patch sticks out of the coarse domain
+
+
+@pytest.mark.parametrize("ratio", [2, 4])
+def test_average_down_is_exact_for_linear_data_and_conserves(ratio):
+    wc, wf = levels(ratio=ratio, bc_c=W.OUTFLOW, lo=(4, 2, 6), patch=(8, 4, 6), nbox_f=None)
+    wf.params["nbox"] = [wf.params["ndom"][0] // 2, wf.params["ndom"][1], wf.params["ndom"][2] // 2]     # 2 x 1 x 2 fine boxes
+    pc, pf = O.make_params(wc.params), O.make_params(wf.params)
+    # fine data = a dyadic linear field at the fine centres: the mean of the children is the field at the parent centre
+    f = lambda c, x, y, z: (1 + c) * 0.25 + 2.0 * x - 0.75 * y + 1.5 * z
+    nf = wf.params["ndom"]
+    xs = [(np.arange(nf[d]) + 0.5) * wf.dx[d] + wf.params["prob_lo"][d] for d in range(3)]
+    Gf = np.stack([f(c, xs[0][None, None, :], xs[1][None, :, None], xs[2][:, None, None]) * np.ones((nf[2], nf[1], nf[0]))
+                   for c in range(wf.nvar)])
+    Uf = W.scatter_valid(wf, Gf, ghost_value=np.nan)
+    Uc = W.scatter_valid(wc, np.full((wc.nvar, 16, 16, 16), -7.0), ghost_value=np.nan)
+    O.average_down(pc, Uc, pf, Uf, (4, 2, 6), ratio)
+    Gc = W.gather_valid(wc, Uc)
+    xc = [(np.arange(16) + 0.5) * wc.dx[d] for d in range(3)]
+    exact = np.stack([f(c, xc[0][None, None, :], xc[1][None, :, None], xc[2][:, None, None]) * np.ones((16, 16, 16))
+                      for c in range(wc.nvar)])
+    patch = (slice(None), slice(6, 12), slice(2, 6), slice(4, 12))
+    assert np.array_equal(Gc[patch], exact[patch])
+    outside = np.ones((16, 16, 16), bool)
+    outside[patch[1:]] = False
+    assert np.all(Gc[:, outside] == -7.0)                               # nothing outside the patch is touched
+    # conservation with random fine data: coarse total over the patch == fine total
+    rng = np.random.default_rng(9)
+    Gr = rng.standard_normal(Gf.shape)
+    Uf = W.scatter_valid(wf, Gr, ghost_value=np.nan)
+    O.average_down(pc, Uc, pf, Uf, (4, 2, 6), ratio)
+    Gc = W.gather_valid(wc, Uc)
+    for c in range(wc.nvar):
+        assert Gc[c][patch[1:]].sum() * np.prod(wc.dx) == pytest.approx(Gr[c].sum() * np.prod(wf.dx), rel=1e-13, abs=1e-15)
