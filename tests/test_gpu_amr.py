@@ -112,4 +112,4 @@ def test_average_down_bit_for_bit(ratio):
     hc.upload(Uc, 1); hf.upload(Uf, 0)
     hc.hydro_average_down(1, hf, 0, (4, 2, 6), ratio)
     O.average_down(O.make_params(wc.params), Uc, O.make_params(wf.params), Uf, (4, 2, 6), ratio)
-    assert np.array_equal(hc.download(1), Uc, equal_nan=True)
+    assert np.array_equal(hc.download(1).reshape(Uc.shape), Uc, equal_nan=True)
