@@ -36,6 +36,9 @@
  * rho*e_1 = rho*e_0 (1 + gamma A dt) after one stage and the Heun closed form after two -- fixes the sign
  * of p_c div(u_face), the state p_c is taken from and every direction's dxinv; P15: a step in e moved by
  * the upwinded mass flux only -- fixes the side F_e takes e from).
+ * The CTU update O12 (oracle_ctu_step, readings C1-C9 further down; pins P16-P22 in tests/test_oracle_ctu.py) and the
+ * two-level ghost fill / restriction O13 (oracle_fill_from_coarse, oracle_average_down, readings A1-A6; pins in
+ * tests/test_oracle_amr.py) carry their readings and pin lists in their own headers below.
  * Parity unpinned: behaviour when the small_dens / small_pres floors trigger
  * (exercised GPU-vs-oracle only).
  *
