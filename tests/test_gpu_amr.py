@@ -113,3 +113,39 @@ def test_average_down_bit_for_bit(ratio):
     hc.hydro_average_down(1, hf, 0, (4, 2, 6), ratio)
     O.average_down(O.make_params(wc.params), Uc, O.make_params(wf.params), Uf, (4, 2, 6), ratio)
     assert np.array_equal(hc.download(1).reshape(Uc.shape), Uc, equal_nan=True)
+
+
+def test_two_level_driver_three_steps_against_the_oracle():
+    """paper_2007_05218_b200/amr.py: three RK2 steps of a coarse level with a 2x-refined patch on its reflecting
+    floor (config-4 recipe: gravity, 2 species), fill_from_coarse at both stages and average_down after every
+    step, against the same sequence of oracle calls."""
+    from paper_2007_05218_b200 import amr
+    from parity_util import rel_err
+    wc = W.config(4, ndom=(32, 32, 32), nbox=(16, 16, 16), nspec=2)
+    lo, extent, ratio = (8, 8, 0), (16, 16, 8), 2
+    tl = amr.TwoLevelHydro(wc.params, lo, extent, ratio, (16, 16, 16))
+    assert tl.fine_params["bc_lo"] == [EXT, EXT, W.REFLECT] and tl.fine_params["bc_hi"] == [EXT, EXT, EXT]
+    wf = W.Workload("patch", wc.kind, tl.fine_params, 1, seed=wc.seed, extra=wc.extra)
+    Uc = W.initial_state(wc)
+    Gc = W.gather_valid(wc, Uc)
+    Gf = np.repeat(np.repeat(np.repeat(Gc[:, 0:8, 8:24, 8:24], 2, axis=1), 2, axis=2), 2, axis=3)
+    Uf = W.scatter_valid(wf, Gf, ghost_value=np.nan)
+    tl.coarse.upload(Uc, 0); tl.fine.upload(Uf, 0)
+    pc, pf = O.make_params(wc.params), O.make_params(tl.fine_params)
+    Uc1, Uf1 = np.zeros_like(Uc), np.zeros_like(Uf)
+    for _ in range(3):
+        dt_o = min(O.estimate_dt(pc, Uc), O.estimate_dt(pf, Uf))
+        for stage in (0, 1):
+            sc, sf = (Uc, Uf) if stage == 0 else (Uc1, Uf1)
+            O.fill_ghosts(pc, sc); O.fill_ghosts(pf, sf)
+            O.fill_from_coarse(pf, sf, pc, sc, lo, ratio)
+            O.advance_stage(pc, stage, dt_o, Uc, Uc1); O.advance_stage(pf, stage, dt_o, Uf, Uf1)
+        O.average_down(pc, Uc, pf, Uf, lo, ratio)
+        dt = tl.step()
+        assert abs(dt - dt_o) <= 1e-12 * dt_o
+    assert np.all(rel_err(wc, tl.coarse.download(0).reshape(Uc.shape), Uc) <= 1e-11)
+    assert np.all(rel_err(wf, tl.fine.download(0).reshape(Uf.shape), Uf) <= 1e-11)
+    # the coarse zones under the patch are the means of their children
+    Gc2, Gf2 = W.gather_valid(wc, Uc), W.gather_valid(wf, Uf)
+    kids = Gf2.reshape(wf.nvar, 8, 2, 16, 2, 16, 2).mean(axis=(2, 4, 6))
+    assert np.allclose(Gc2[:, 0:8, 8:24, 8:24], kids, rtol=1e-14, atol=1e-15)
