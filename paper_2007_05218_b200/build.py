@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhydro_b200.so")
 PROBE_LIB = os.path.join(HERE, "libhydro_probe_b200.so")
 SOURCES = ["hydro_api.cu"]
-HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_yz.cuh", "march_ring.cuh", "march_x.cuh", "ctu.cuh", "amr_fill.cuh", "ghost_reduce.cuh",
+HEADERS = ["hydro_device.cuh", "sweep_x.cuh", "sweep_xc.cuh", "sweep_yz.cuh", "march_ring.cuh", "march_x.cuh", "ctu.cuh", "amr_fill.cuh", "ghost_reduce.cuh",
            "flatten.cuh"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo"]
 

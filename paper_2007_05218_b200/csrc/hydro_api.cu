@@ -15,6 +15,7 @@
 #include "flatten.cuh"
 #include "hydro_device.cuh"
 #include "sweep_x.cuh"
+#include "sweep_xc.cuh"
 #include "sweep_yz.cuh"
 #include "march_ring.cuh"
 #include "march_x.cuh"
@@ -56,7 +57,7 @@ struct Carve {
 
 // tuning switches, read from the environment ONCE per hydro_init (include/hydro.h lists them)
 struct Knobs {
-    int ring, seglen, nsmax, fuse_dt, split_ghosts, fill_monolithic, xmarch, species_one_launch;
+    int ring, seglen, nsmax, fuse_dt, split_ghosts, fill_monolithic, xmarch, species_one_launch, xchunk;
 };
 
 int env_int(const char *name, int dflt)
@@ -98,7 +99,8 @@ struct hydro_ctx {
     CUtensorMap maps[2][2][7]; // [state][DIR-1][components per box]: TMA views of the states for the ring kernels
     CUtensorMap fmaps[2];      // [DIR-1]: TMA views of the flattening-coefficient array (flatten == 1)
     bool external;             // some face is HYDRO_BC_EXTERNAL (sharded MultiFab)
-    bool use_xmarch;           // x sweep by the marching kernels of march_x.cuh (else k_sweep_x)
+    bool use_xmarch;           // x sweep by the marching kernels of march_x.cuh (else k_sweep_xc / k_sweep_x)
+    bool use_xchunk;           // x sweep by the chunk-lane kernel of sweep_xc.cuh (else k_sweep_x)
     CUtensorMap xmaps[2][6];   // [state][components per box]: {4 zones, 128 rows} views for the x hydro marching kernel
     CUtensorMap xsmaps[2][6];  // the same with XS_ROWS rows per box, for the x species marching kernels
     CUtensorMap fxmap;         // {4 columns, XS_ROWS rows} view of the face mass-flux array in its x layout (rows of nb0 + 4)
@@ -594,6 +596,18 @@ int advance_stage_impl(hydro_handle h, int stage, double dt, const double *dt_de
     if (h->use_xmarch) {   // x sweep: a thread per row, marching (march_x.cuh)
         int rc = xmarch_stage(h, stage, a.Lacc, a.Frho);
         if (rc) return rc;
+    } else if (h->use_xchunk) {   // x sweep: a lane per 4-zone chunk of the flattened valid rows (sweep_xc.cuh)
+        const long long T = (long long)g.nb[1] * g.nb[2] * (g.nt[0] / 4);
+        const long long warps = (T + XC_LANES - 1) / XC_LANES;
+        const unsigned gy = g.nboxes < 32768 ? g.nboxes : 32768, gz = (g.nboxes + gy - 1) / gy;
+        const dim3 xg((unsigned)((warps + XC_WARPS - 1) / XC_WARPS), gy, gz);
+        prof_begin(h);
+        if (g.flatten && g.evolve) k_sweep_xc<true, true><<<xg, XC_WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
+        else if (g.flatten) k_sweep_xc<true, false><<<xg, XC_WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, a.FL);
+        else if (g.evolve) k_sweep_xc<false, true><<<xg, XC_WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
+        else k_sweep_xc<false, false><<<xg, XC_WARPS * 32, 0, h->stream>>>(g, a.Us, a.Lacc, nullptr);
+        int rc = check_launch(h, "k_sweep_xc", K_SWEEP_X);
+        if (rc) return rc;
     } else {   // x sweep: one warp per 26-zone chunk of a row
         constexpr int WARPS = 4;
         const int nchunk = (g.nb[0] + XW_VALID - 1) / XW_VALID;
@@ -830,6 +844,7 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
     h->kn.fill_monolithic = env_int("HYDRO_FILL_MONOLITHIC", 0);
     h->kn.xmarch = env_int("HYDRO_XMARCH", 0);
     h->kn.species_one_launch = env_int("HYDRO_SPECIES_ONE_LAUNCH", 1);
+    h->kn.xchunk = env_int("HYDRO_XCHUNK", 1);
     h->ns_max = (h->kn.nsmax >= 1 && h->kn.nsmax <= NS_MAX) ? h->kn.nsmax : NS_MAX;
     for (int d = 0; d < 3; ++d) h->seglen[d] = d == 0 ? g.nb[0] : pick_seglen(g, d, h->kn.seglen);
     {   // TMA tensor copies: 16-byte row pitch AND 16-byte aligned box starts (the first valid zone of a row sits
@@ -861,6 +876,12 @@ int hydro_init(const hydro_params *p, void *U0_dev, void *U1_dev, void *scratch_
             if (!make_fx_map(&h->fxmap, (double *)(h->scratch + cv.frho), g, XS_ROWS, why2)) h->use_xmarch = false;
         }
     }
+    // chunk-lane x sweep (sweep_xc.cuh): whole 4-zone chunks (256-bit loads and stores: 32-byte aligned arrays), the
+    // flattened chunk sequence of a box in an int
+    h->use_xchunk = h->kn.xchunk != 0 && g.ng % 4 == 0 && g.nb[0] % 4 == 0 &&
+                    (long long)g.nb[1] * g.nb[2] * (g.nt[0] / 4) < (1LL << 30) &&
+                    ((uintptr_t)U0_dev % 32) == 0 && ((uintptr_t)U1_dev % 32) == 0 && ((uintptr_t)(h->scratch + cv.lacc) % 32) == 0 &&
+                    (!g.flatten || ((uintptr_t)(h->scratch + cv.flat) % 32) == 0);
     cudaError_t e = cudaSuccess;
     if (g.flatten) {   // coefficient array = 1 (no flattening) outside the zones k_flatten writes
         double *FL = (double *)(h->scratch + cv.flat);
@@ -1099,6 +1120,7 @@ int hydro_query(hydro_handle h, int what)
         case 3: return h->ns_max;
         case 4: return h->use_xmarch ? 1 : 0;
         case 5: return h->use_ring ? (h->kn.species_one_launch & 3) : 0;
+        case 6: return (!h->use_xmarch && h->use_xchunk) ? 1 : 0;
         default: return -1;
     }
 }

@@ -24,6 +24,7 @@ for name, make in CASES:
         wl = make()
         wl.params.update(opts)
         h = Hydro(wl.params)
+        assert h.hydro_query(6) == (0 if name == "cfg3_odd_box" else 1), name   # chunk-lane x sweep where the rows allow
         U0 = W.initial_state(wl)
         h.upload(U0, 0)
         p = O.make_params(wl.params)
@@ -51,8 +52,28 @@ for name, make in CASES[:3]:
     print(name, "xmarch", "bitwise" if ok else "DIFFERS", flush=True)
     if not ok:
         bad.append((name, "xmarch"))
-# the CTU update O12: strict build == oracle_ctu_step, bit for bit
 os.environ["HYDRO_XMARCH"] = "0"
+# the one-zone-per-lane x sweep (k_sweep_x, HYDRO_XCHUNK=0; the default on these geometries is the chunk-lane
+# kernel of sweep_xc.cuh, exercised by the first loop): bitwise too, with and without the options
+os.environ["HYDRO_XCHUNK"] = "0"
+for name, make in CASES[:3]:
+    for opts in ({}, {"flatten": 1, "evolve_eint": 1}):
+        wl = make()
+        wl.params.update(opts)
+        h = Hydro(wl.params)
+        assert h.hydro_query(6) == 0, name
+        U0 = W.initial_state(wl)
+        h.upload(U0, 0)
+        p = O.make_params(wl.params)
+        Uo, T = U0.copy(), np.zeros_like(U0)
+        dts_o = [O.step(p, Uo, T) for _ in range(3)]
+        dts_g = h.hydro_step(3, all_dts=True)
+        ok = dts_o == dts_g and np.array_equal(W.gather_valid(wl, h.download(0).reshape(U0.shape)), W.gather_valid(wl, Uo))
+        print(name, opts, "k_sweep_x", "bitwise" if ok else "DIFFERS", flush=True)
+        if not ok:
+            bad.append((name, "k_sweep_x"))
+os.environ["HYDRO_XCHUNK"] = "1"
+# the CTU update O12: strict build == oracle_ctu_step, bit for bit
 for name, make in CASES:
     wl = make()
     h = Hydro(wl.params)
