@@ -32,6 +32,9 @@
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 
+#ifndef RING_UNROLL_S
+#define RING_UNROLL_S 1     // unroll of the march loop of the species kernels
+#endif
 #ifndef RING_UNROLL_Z
 #define RING_UNROLL_Z 1     // unroll of the march loop of the FINAL hydro kernels (2 spills at 168 registers)
 #endif
@@ -439,6 +442,8 @@ __device__ __forceinline__ void march_species_body(const Geom& g, const SweepArg
     double Fnext = 0.0;
     double f1 = 1.0, f2 = 1.0;               // O10 coefficients of zones n-1, n-2 (FLAT)
 
+    constexpr int UNROLL_S = RING_UNROLL_S;
+#pragma unroll UNROLL_S
     for (int it = 0; it < nsteps; ++it, lz += lmstride, fz += lmstride, zo += mstride) {
         const bool upd = (it >= 6);
         const double Frho = Fnext;
