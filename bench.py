@@ -330,6 +330,7 @@ def run_ours(args, rank, world, local_rank):
     launches0 = h.hydro_launch_count()
     ns_max, split_ghosts, fuse_dt = h.hydro_query(3), bool(h.hydro_query(1)), bool(h.hydro_query(2))
     xmarch = bool(h.hydro_query(4))
+    xchunk = bool(h.hydro_query(6))
     one_launch = max(0, h.hydro_query(5))
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -446,7 +447,7 @@ def run_ours(args, rank, world, local_rank):
     if rank == 0:
         cfg = workload_config(wl, args.config)
         cfg.update({"replicas": world, "host_generation_s": round(t_gen, 1), "species_groups_yz": groups,
-                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt, "x_sweep": "marching (march_x.cuh)" if xmarch else "lane-parallel (sweep_x.cuh)", "species_groups_in_one_launch": {"y": bool(one_launch & 1), "z": bool(one_launch & 2)},
+                    "flatten": bool(wl.params.get("flatten", 0)), "evolve_eint": bool(wl.params.get("evolve_eint", 0)), "split_ghost_fill": split_ghosts, "dt_fused_in_z_sweep": fuse_dt, "x_sweep": "marching (march_x.cuh)" if xmarch else ("chunk-lane (sweep_xc.cuh)" if xchunk else "one zone per lane (sweep_x.cuh)"), "species_groups_in_one_launch": {"y": bool(one_launch & 1), "z": bool(one_launch & 2)},
                     "call": f"hydro_step(h, {args.steps}) -- one C-ABI call for the K timed steps",
                     "fmad": open(B.LIB_PATH + ".flags").read() if os.path.exists(B.LIB_PATH + ".flags") else "?"})
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

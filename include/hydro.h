@@ -94,8 +94,11 @@ size_t hydro_scratch_bytes(const hydro_params *p);
  * Tuning switches, read from the environment ONCE, here (they select among internal code paths
  * that give bit-identical results; defaults in brackets; hydro_query reports what a handle uses):
  *   HYDRO_RING=0            plain-load y/z sweeps instead of the TMA-ring marching kernels   [1]
- *   HYDRO_XMARCH=1          x sweep by the thread-per-row marching kernels of march_x.cuh instead of the
- *                           lane-parallel k_sweep_x (measured equal in time, profiles/r02_xmarch.md)  [0]
+ *   HYDRO_XCHUNK=0          x sweep by the one-zone-per-lane k_sweep_x (sweep_x.cuh) instead of the chunk-lane
+ *                           k_sweep_xc (sweep_xc.cuh: a lane owns a 4-zone chunk; taken where ng and nbox[0]
+ *                           are multiples of 4 and the buffers are 32-byte aligned; profiles/r02_xchunk.md)  [1]
+ *   HYDRO_XMARCH=1          x sweep by the thread-per-row marching kernels of march_x.cuh instead of either
+ *                           (measured equal in time to k_sweep_x, profiles/r02_xmarch.md)    [0]
  *   HYDRO_SEGLEN=n          zones per pencil segment of the y/z sweeps                       [auto]
  *   HYDRO_NSMAX=n           passive species per thread and launch, 1..5                      [5]
  *   HYDRO_SPECIES_ONE_LAUNCH=m  bit 0: the y species sweep, bit 1: the z species sweep launches all species groups
@@ -194,9 +197,10 @@ int hydro_average_down(hydro_handle coarse, int which_coarse, hydro_handle fine,
  *           copies) instead of one k_fill_ghosts launch per stage;
  *        2: hydro_step reduces the next step's dt inside the stage-1 z hydro sweep;
  *        3: passive species per thread and launch in the species sweeps;
- *        4: the x sweep runs as marching kernels (a thread per row, march_x.cuh; 1) or as the
- *           lane-parallel k_sweep_x (0);
- *        5: which species sweeps launch all species groups together (bit 0: y, bit 1: z).
+ *        4: the x sweep runs as marching kernels (a thread per row, march_x.cuh; 1) or as a
+ *           lane-parallel kernel (0: see 6);
+ *        5: which species sweeps launch all species groups together (bit 0: y, bit 1: z);
+ *        6: the lane-parallel x sweep is the chunk-lane k_sweep_xc (1) or the one-zone-per-lane k_sweep_x (0).
  * Returns -1 for a NULL handle or an unknown `what`. */
 int hydro_query(hydro_handle h, int what);
 
