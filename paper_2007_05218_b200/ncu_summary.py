@@ -22,7 +22,7 @@ N_SM = 148
 
 
 # the kernel sources of the RK2 path's default launches (the classes of hydro_profile_read 0..8)
-PATH_SOURCES = ["flatten.cuh", "ghost_reduce.cuh", "hydro_device.cuh", "march_ring.cuh", "sweep_x.cuh", "sweep_yz.cuh"]
+PATH_SOURCES = ["flatten.cuh", "ghost_reduce.cuh", "hydro_device.cuh", "march_ring.cuh", "sweep_x.cuh", "sweep_xc.cuh", "sweep_yz.cuh"]
 
 
 def source_sha() -> str:
@@ -118,15 +118,81 @@ def summarise(launches):
     return classes
 
 
+def read_launch_list(path):
+    """`ncu --metrics gpu__time_duration.sum --csv --log-file` (one row per launch and metric) -> [(kernel, ms)]."""
+    rows = [r for r in csv.reader(open(path)) if len(r) > 10]
+    hdr = rows[0]
+    ik, im, iu, iv = hdr.index("Kernel Name"), hdr.index("Metric Name"), hdr.index("Metric Unit"), hdr.index("Metric Value")
+    out = []
+    for r in rows[1:]:
+        if r[im] != "gpu__time_duration.sum":
+            continue
+        name = re.sub(r"^void |\(.*$", "", r[ik]).replace("hydro::", "")
+        out.append((name, num(r[iv]) * UNIT.get(r[iu], 1.0)))
+    return out
+
+
+def final_report(launch_csv, bench_json, md, title, command):
+    """The end-of-round record: the ncu launch list of a bench.py run (per-kernel means and shares of the step)
+    beside the live CUDA-event classes of the bench line (json.loads of bench.py's one line of output)."""
+    L = read_launch_list(launch_csv)
+    per = {}
+    for name, ms in L:
+        per.setdefault(name, []).append(ms)
+    step = {k: v for k, v in per.items() if classify(k)[0] in ("sweep_x", "fill_ghosts", "estimate_dt", "hydro_y", "hydro_z", "species_y", "species_z", "flatten")}
+    tot = sum(sum(v) for v in step.values())
+    b = json.load(open(bench_json))
+    with open(md, "w") as f:
+        f.write(f"# {title}\n\nCommands (B200, committed files only):\n\n```\n{command}\n```\n\n")
+        f.write("ncu per-launch times are cold-cache, serialised and at unthrottled clocks: compare SHARES with the live CUDA-event "
+                "shares of bench.py below (totals and probe kernels, launched after the timed region, are left out of the shares).\n\n")
+        f.write("| kernel | launches | mean ms (ncu) | share (ncu) |\n|---|---|---|---|\n")
+        for k, v in per.items():
+            if "at::" in k:
+                continue
+            sh = f"{sum(v) / tot:.3f}" if k in step else ""
+            f.write(f"| `{k}` | {len(v)} | {sum(v) / len(v):.3f} | {sh} |\n")
+        ncu_cls = {}
+        for k, v in step.items():
+            c = classify(k)[0]
+            ncu_cls[c] = ncu_cls.get(c, 0.0) + sum(v) / tot
+        peak = b["roofline"]["peak"]
+        f.write(f"\nbench.py kernel classes (CUDA events around every launch of a second hydro_step call; `value` is timed without them) "
+                f"beside the ncu class shares; traffic ratio = ncu DRAM bytes (profiles/traffic.json) / algorithmic bytes; issue / FP64 = "
+                f"ncu instruction counts over the live duration against 148 x 4 x the sampled SM clock and the measured FP64 peak:\n\n")
+        f.write(f"| class | ms/launch | launches/step | share of step (events) | share (ncu) | alg GB/launch | GB/s | frac of measured {peak:.0f} | "
+                "traffic ratio | issue slots | FP64 pipe |\n|---|---|---|---|---|---|---|---|---|---|---|\n")
+        fmt = lambda x, n=3: "" if x is None else f"{x:.{n}f}"
+        for k, v in b["kernels"].items():
+            f.write(f"| {k} | {v['ms_per_launch']:.3f} | {v['launches_per_step']:.1f} | {v['share_of_step']:.3f} | {fmt(ncu_cls.get(k))} | "
+                    f"{v['alg_gb_per_launch']:.2f} | {v['gbs']:.0f} | {v['frac']:.3f} | {fmt(v.get('traffic_ratio'))} | "
+                    f"{fmt(v.get('issue_slot_frac'))} | {fmt(v.get('fp64_pipe_frac'))} |\n")
+        ws = b["roofline"]["whole_step"]
+        f.write(f"\nbench line: value {b['value']:.4g} {b['unit']}, {b['ms_per_step']:.2f} ms/step, {b['gpu_launches']} launches in the timed "
+                f"region, whole step {ws['alg_bytes_per_zone_update']:.0f} B/zone-update = {ws['gbs']:.0f} GB/s = {ws['frac']:.3f} of measured / "
+                f"{ws['frac_of_nominal_8000']:.3f} of nominal 8000; dominant class {b['roofline']['kernel']} at {b['roofline']['frac']:.3f} of the "
+                f"HBM peak; clocks {b['clocks']}; ")
+        cb, e2e = b.get("cpu_baseline"), b.get("e2e")
+        if cb:
+            f.write(f"cpu_baseline {cb['value']:.4g} on {cb['cores']} cores" + (f", {cb['one_core']['value']:.4g} on one" if cb.get("one_core") else "") + "; ")
+        if e2e:
+            f.write(f"e2e {e2e['value']:.4g} ({e2e['seconds_per_call']:.2f} s per {e2e['steps']}-step host-buffer call).")
+        f.write("\n\nFull JSON line:\n\n```\n" + json.dumps(b) + "\n```\n")
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("raw")
+    ap.add_argument("raw", help="ncu --page raw --csv export, or with --final the launch-list csv")
+    ap.add_argument("--final", metavar="BENCH_JSON", help="write the end-of-round record (--md) from a launch list and a bench line")
     ap.add_argument("--config", default="cfg5_scaling")
     ap.add_argument("--json")
     ap.add_argument("--md")
     ap.add_argument("--command", default="")
     ap.add_argument("--title", default="ncu --set full, one whole RK2 step")
     a = ap.parse_args()
+    if a.final:
+        final_report(a.raw, a.final, a.md, a.title, a.command)
+        return
     launches = read_raw(a.raw)
     classes = summarise(launches)
     if a.json:
