@@ -34,6 +34,14 @@ constexpr int BS = 128;               // threads per CTA of the marching kernels
 #define HYDRO_RING_D 8
 #endif
 constexpr int RING_D = HYDRO_RING_D;  // depth of the TMA ring of the marching kernels
+#ifndef HYDRO_RING_D_SY
+#define HYDRO_RING_D_SY 6
+#endif
+#ifndef HYDRO_RING_D_SZ
+#define HYDRO_RING_D_SZ 6
+#endif
+// depth of the ring of the species kernels, y sweep (not FINAL) and z sweep (FINAL)
+constexpr int ring_ds(bool final_) { return final_ ? HYDRO_RING_D_SZ : HYDRO_RING_D_SY; }
 #ifndef HYDRO_XM_D
 #define HYDRO_XM_D 3
 #endif
@@ -335,11 +343,19 @@ void set_smem(hydro_handle h, K kernel, size_t bytes)
     h->configured.insert((const void *)kernel);
 }
 
+// bytes of the accumulator prefetch ring of the species march kernels (march_ring.cuh, RING_LPD)
+constexpr size_t lring_bytes(int n, bool final_, int stage)
+{
+    const int lpd = final_ ? RING_LPD_Z : RING_LPD_Y;
+    return lpd ? (size_t)(lpd + 1) * n * ((final_ && stage == 1) ? 2 : 1) * BS * 8 : 0;
+}
+
 template <int DIR, bool FINAL, int STAGE, int N, bool FLAT>
 void launch_species_ring_n(hydro_handle h, const SweepArgs &a, dim3 grid, const RingMaps &tm)
 {
-    const size_t sm = (size_t)RING_D * (1 + N + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
-    auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, RING_D, FLAT>;
+    constexpr int DS = ring_ds(FINAL);
+    const size_t sm = (size_t)DS * (1 + N + (FLAT ? 1 : 0)) * BS * 8 + DS * 8 + lring_bytes(N, FINAL, STAGE);
+    auto kern = k_march_species<DIR, FINAL, STAGE, N, BS, DS, FLAT>;
     set_smem(h, kern, sm);
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
@@ -347,8 +363,9 @@ void launch_species_ring_n(hydro_handle h, const SweepArgs &a, dim3 grid, const 
 template <int DIR, bool FINAL, int STAGE, bool FLAT>
 void launch_energy_ring(hydro_handle h, const SweepArgs &a, dim3 grid, const RingMaps &tm)
 {
-    const size_t sm = (size_t)RING_D * (2 + (FLAT ? 1 : 0)) * BS * 8 + RING_D * 8;
-    auto kern = k_march_species<DIR, FINAL, STAGE, 1, BS, RING_D, FLAT, FINAL>;   // ENERGY terms only in the FINAL sweep
+    constexpr int DS = ring_ds(FINAL);
+    const size_t sm = (size_t)DS * (2 + (FLAT ? 1 : 0)) * BS * 8 + DS * 8 + lring_bytes(1, FINAL, STAGE);
+    auto kern = k_march_species<DIR, FINAL, STAGE, 1, BS, DS, FLAT, FINAL>;   // ENERGY terms only in the FINAL sweep
     set_smem(h, kern, sm);
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
@@ -382,13 +399,14 @@ void launch_species_groups(hydro_handle h, const SweepArgs &a, int nsa, dim3 gri
     tm.b2 = h->maps[state][DIR - 1][nsa > 1 ? nsa - 1 : 1];
     tm.f = h->fmaps[DIR - 1];
     const bool flat = h->g.flatten != 0;
-    const size_t sm = (size_t)RING_D * (1 + nsa + (flat ? 1 : 0)) * BS * 8 + RING_D * 8;
+    constexpr int DS = ring_ds(FINAL);
+    const size_t sm = (size_t)DS * (1 + nsa + (flat ? 1 : 0)) * BS * 8 + DS * 8 + lring_bytes(nsa, FINAL, STAGE);
     grid.x *= a.ngroups;
     switch (nsa) {
 #define CASE(N) case N: \
-        if (flat) { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, RING_D, true>; set_smem(h, kern, sm); \
+        if (flat) { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, DS, true>; set_smem(h, kern, sm); \
                     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } \
-        else { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, RING_D, false>; set_smem(h, kern, sm); \
+        else { auto kern = k_march_species_groups<DIR, FINAL, STAGE, N, BS, DS, false>; set_smem(h, kern, sm); \
                kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm); } \
         break;
         CASE(2) CASE(3) CASE(4) CASE(5)

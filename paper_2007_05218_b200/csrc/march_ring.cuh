@@ -32,6 +32,15 @@
 #define RING_MINB_S 4      // same for the species kernels (NS <= 5 species per thread fit 128 registers)
 #endif
 
+// species kernels: march steps by which the accumulator (and U0) values of a zone are fetched ahead through a
+// per-thread cp.async ring in shared memory (0: plain loads at the top of the zone's own step); y sweep (not FINAL) and
+// z sweep (FINAL) separately: the ring costs shared memory, which the z kernels (KEEP slots) cannot spare
+#ifndef RING_LPD_Y
+#define RING_LPD_Y 1
+#endif
+#ifndef RING_LPD_Z
+#define RING_LPD_Z 0
+#endif
 #ifndef RING_UNROLL_S
 #define RING_UNROLL_S 1     // unroll of the march loop of the species kernels
 #endif
@@ -395,6 +404,12 @@ __device__ __forceinline__ void march_species_body(const Geom& g, const SweepArg
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* ring = reinterpret_cast<double*>(smem_raw);
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)D * NROW * BS * 8);
+    // accumulator / U0 values of the zone updated LPD steps from now, one double per thread and species: each thread
+    // copies and reads back its own values only (cp.async, completion in order: no barrier, no registers held)
+    constexpr int LPD = FINAL ? RING_LPD_Z : RING_LPD_Y, LSL = LPD + 1;
+    constexpr bool UB = FINAL && STAGE == 1;
+    constexpr int NL = NS * (UB ? 2 : 1);
+    double* lring = reinterpret_cast<double*>(smem_raw + (size_t)D * NROW * BS * 8 + (size_t)D * 8);
 
     const int tid = threadIdx.x;
     const int tiles = gx / g.nboxes;
@@ -449,12 +464,31 @@ __device__ __forceinline__ void march_species_body(const Geom& g, const SweepArg
         const double Frho = Fnext;
         if (it >= 4 && it + 1 < nsteps) Fnext = ldg(a.Frho + fz + lmstride);
         double lacc[NS], ubase[NS], ldiv = 0.0, eE = 0.0, rEn = 0.0;
+        if (LPD > 0) {
+            const int itp = it + LPD;
+            if (itp >= 6 && itp < nsteps) {
+                const uint32_t dst = smem_u32(lring + (size_t)(itp % LSL) * NL * BS + tid);
+#pragma unroll
+                for (int v = 0; v < NS; ++v)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + (uint32_t)(v * BS * 8)),
+                                 "l"(a.Lacc + lz + LPD * lmstride + v * g.lcstride) : "memory");
+                if (UB) {
+#pragma unroll
+                    for (int v = 0; v < NS; ++v)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + (uint32_t)((NS + v) * BS * 8)),
+                                     "l"(a.Ubase + zo + LPD * mstride + v * g.cstride) : "memory");
+                }
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        }
         if (upd) {
+            if (LPD == 0) {
 #pragma unroll
-            for (int v = 0; v < NS; ++v) lacc[v] = a.Lacc[lz + v * g.lcstride];
-            if (FINAL && STAGE == 1) {
+                for (int v = 0; v < NS; ++v) lacc[v] = a.Lacc[lz + v * g.lcstride];
+                if (UB) {
 #pragma unroll
-                for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo + v * g.cstride];
+                    for (int v = 0; v < NS; ++v) ubase[v] = a.Ubase[zo + v * g.cstride];
+                }
             }
             if (ENERGY) {     // div(u_face) and rho*E - K left by the z hydro kernel, and the new rho*E
                 ldiv = a.Lacc[lz + g.lcstride];
@@ -485,6 +519,16 @@ __device__ __forceinline__ void march_species_body(const Geom& g, const SweepArg
         f2 = f1; f1 = fn;
         // pass 2: accumulator / stage update (first use of this step's global loads)
         if (upd) {
+            if (LPD > 0) {
+                asm volatile("cp.async.wait_group %0;" ::"n"(LPD) : "memory");
+                const double* src = lring + (size_t)(it % LSL) * NL * BS + tid;
+#pragma unroll
+                for (int v = 0; v < NS; ++v) lacc[v] = src[v * BS];
+                if (UB) {
+#pragma unroll
+                    for (int v = 0; v < NS; ++v) ubase[v] = src[(NS + v) * BS];
+                }
+            }
 #pragma unroll
             for (int v = 0; v < NS; ++v) out[v] = lacc[v] - out[v] * dinv;
             if (FINAL) {
