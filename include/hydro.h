@@ -233,6 +233,46 @@ const char *hydro_last_error(hydro_handle h);
 int hydro_run_host(const hydro_params *p, double *U_host, int nsteps, double *dt_host,
                    double *totals_host);
 
+/* O9 totals (the sums of hydro_conserved_totals, bit for bit) for a caller that has a state on the device but may not
+ * allocate anything: no handle, no scratch buffer, no pinned memory.
+ *
+ * Who that is: the codes of the paper draw all device memory from a pool that is grabbed up front and handed out as
+ * sub-buffers, because cudaMalloc inside the timestep loop is "disastrous".  A diagnostics routine, an
+ * in-situ monitor or a plug-in that is called from inside such a code is lent a pointer to the state and nothing
+ * else: it has no access to the host code's pool, a cudaMalloc of its own may simply fail because the pool has
+ * already taken the device's memory, and where it succeeds it stalls the device in the middle of a step.  Such a
+ * caller cannot build a handle either (hydro_init wants a scratch buffer and pins host memory).  This call needs
+ * neither: the partial sums of the reduction live in an array compiled into the library.
+ *
+ *   p           HOST: describes the state (ndom, nbox, ng, nspec, prob_lo/hi must be valid; the rest is ignored
+ *               beyond the usual validation).
+ *   U_dev       DEVICE, read only: one state in layout a1, hydro_state_bytes(p) bytes, 8-byte aligned.
+ *   totals_dev  DEVICE, written: NFLUX = 5 + nspec doubles, 8-byte aligned, on the same device as U_dev;
+ *               totals_dev[f] = sum over valid zones of conserved component f times dx*dy*dz.
+ *   cuda_stream a cudaStream_t of that device (NULL = legacy default stream).  The two kernels are enqueued on it
+ *               and the call returns without waiting; read totals_dev after synchronising that stream.
+ *
+ * Limit: nspec <= HYDRO_TOTALS_STATIC_MAX_NFLUX - 5 = 27.  A larger nspec returns HYDRO_ENOMEM and the message says
+ * what the limit is; use hydro_conserved_totals, whose scratch the caller sizes, for those.  The number of zones
+ * and boxes is not limited.  The built-in array is 592 KiB (32 components x 1184 blocks x 2 doubles); every GPU on
+ * which the library's module is loaded holds its own copy until the process exits, whether or not this call is used.
+ *
+ * First call on a device: looks up the device address of the built-in array (once per device; it can make the CUDA
+ * runtime load the library's module on that device).  Make that first call during start-up, outside any stream
+ * capture; later calls only validate their arguments and launch.
+ *
+ * Sharing: every call on a device uses the same array, on whatever stream it is given.  Two calls that can run on
+ * the GPU at the same time (different streams, or different host threads using different streams) overwrite each
+ * other's partial sums and both may return wrong totals; order them on one stream or with events.  Calls that run
+ * one after the other need no clean-up in between: the first kernel writes every partial sum the second reads, so
+ * the contents left by an earlier call, of any shape, are never seen and nothing has to start at zero.
+ *
+ * Allocates nothing, on the host side of CUDA or on the device: no cudaMalloc / cudaFree / cudaMallocHost, no event
+ * or stream creation, no library call that allocates.  Errors as everywhere: 0 or a negative HYDRO_E* code, message
+ * via hydro_last_error(NULL). */
+#define HYDRO_TOTALS_STATIC_MAX_NFLUX 32
+int hydro_conserved_totals_static(const hydro_params *p, const void *U_dev, void *totals_dev, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,8 @@ HYDRO_OK, HYDRO_EINVAL, HYDRO_ENOMEM, HYDRO_ECUDA, HYDRO_ESTATE = 0, -1, -2, -3,
 EXPORTS = ["hydro_state_bytes", "hydro_scratch_bytes", "hydro_init", "hydro_fill_ghosts",
            "hydro_advance_stage", "hydro_estimate_dt", "hydro_conserved_totals", "hydro_step",
            "hydro_launch_count", "hydro_query", "hydro_profile", "hydro_profile_read", "hydro_destroy", "hydro_last_error", "hydro_run_host",
-           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo", "hydro_ctu_scratch_bytes", "hydro_ctu_step", "hydro_fill_from_coarse", "hydro_average_down"]
+           "hydro_halo_bytes", "hydro_pack_halo", "hydro_unpack_halo", "hydro_ctu_scratch_bytes", "hydro_ctu_step", "hydro_fill_from_coarse", "hydro_average_down",
+           "hydro_conserved_totals_static"]
 PROBE_LIB_PATH = os.path.join(HERE, "libhydro_probe_b200.so")
 PROBE_EXPORTS = ["hydro_probe_fp64"]
 
@@ -94,6 +95,7 @@ def lib():
     L.hydro_halo_bytes.argtypes = [pp, C.c_int]
     L.hydro_pack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
     L.hydro_unpack_halo.argtypes = [vp, C.c_int, C.c_int, C.c_int, vp]
+    L.hydro_conserved_totals_static.argtypes = [pp, vp, vp, vp]
     _lib = L
     return L
 
@@ -112,6 +114,22 @@ def hydro_ctu_scratch_bytes(p: HydroParams) -> int:
 
 def hydro_halo_bytes(p: HydroParams, dim: int) -> int:
     return lib().hydro_halo_bytes(C.byref(p), dim)
+
+
+def hydro_conserved_totals_static(p: HydroParams, U_dev, totals_dev, stream=None):
+    """Conserved totals of a device-resident state for code that must not allocate (include/hydro.h): no handle, no
+    scratch buffer; the reduction's partial sums live in an array built into the library (nspec <= 27).
+
+    U_dev: CUDA float64 tensor holding one state in layout a1; totals_dev: CUDA float64 tensor of 5 + nspec
+    elements on the same device, written by the call; stream: a torch.cuda.Stream of that device (default: the
+    device's current stream).  Asynchronous: synchronise the stream before reading totals_dev.  This wrapper
+    allocates nothing on the device either; both tensors are the caller's."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(U_dev.device)
+    rc = lib().hydro_conserved_totals_static(C.byref(p), U_dev.data_ptr(), totals_dev.data_ptr(), stream.cuda_stream)
+    if rc != 0:
+        raise HydroError(rc, lib().hydro_last_error(None).decode())
 
 
 _probe = None

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <set>
 #include <string>
 #include <vector>
@@ -1222,3 +1223,92 @@ done:
 }
 
 }  // extern "C"
+
+// ---- O9 totals for callers that cannot allocate: hydro_conserved_totals_static (include/hydro.h) ----------------
+// The two-pass reduction of hydro_conserved_totals needs a place for the per-block partial sums.  Every other entry
+// point takes that place from the caller's scratch buffer, which somebody had to cudaMalloc; this one keeps it in
+// the library image instead.  The array below is part of the loaded module: each GPU that loads libhydro_b200.so
+// carries its own 592 KiB copy from the moment the module is loaded there until the process exits, used or not.
+namespace {
+
+constexpr int STATIC_TOTALS_NFLUX = HYDRO_TOTALS_STATIC_MAX_NFLUX;
+constexpr size_t STATIC_TOTALS_DOUBLES = (size_t)STATIC_TOTALS_NFLUX * RED_BLOCKS * 2;   // (hi, lo) per block and component
+
+static __device__ __align__(256) double g_static_partials[STATIC_TOTALS_DOUBLES];
+
+// In host code `g_static_partials` is only a stand-in that the runtime maps to the real array; it is NOT a device
+// address and must never be handed to a kernel.  The device address differs from GPU to GPU, so it is looked up
+// with cudaGetSymbolAddress once per device, with that device current, and remembered here.
+constexpr int STATIC_TOTALS_MAX_DEVICES = 64;
+std::mutex g_static_mutex;
+double *g_static_partials_addr[STATIC_TOTALS_MAX_DEVICES] = {};
+
+}  // namespace
+
+extern "C" int hydro_conserved_totals_static(const hydro_params *p, const void *U_dev, void *totals_dev,
+                                             void *cuda_stream)
+{
+    Geom g; std::string why;
+    if (!make_geom(p, g, why)) return fail(nullptr, HYDRO_EINVAL, why);
+    if (g.nflux > STATIC_TOTALS_NFLUX) {
+        char msg[256];
+        snprintf(msg, sizeof msg,
+                 "hydro_conserved_totals_static: nspec = %d gives %d conserved components, the built-in scratch holds "
+                 "%d (nspec <= %d); use hydro_conserved_totals with a caller-provided scratch buffer instead",
+                 g.nspec, g.nflux, STATIC_TOTALS_NFLUX, STATIC_TOTALS_NFLUX - 5);
+        return fail(nullptr, HYDRO_ENOMEM, msg);
+    }
+    if (!U_dev || !totals_dev) return fail(nullptr, HYDRO_EINVAL, "null U_dev or totals_dev");
+    if (((uintptr_t)U_dev % 8) != 0 || ((uintptr_t)totals_dev % 8) != 0)
+        return fail(nullptr, HYDRO_EINVAL, "U_dev and totals_dev must be 8-byte aligned");
+    int device = -1;
+    {
+        const void *bufs[2] = {U_dev, totals_dev};
+        for (const void *b : bufs) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, b) != cudaSuccess || at.type != cudaMemoryTypeDevice) {
+                cudaGetLastError();
+                return fail(nullptr, HYDRO_EINVAL, "U_dev and totals_dev must be device memory");
+            }
+            if (device >= 0 && at.device != device)
+                return fail(nullptr, HYDRO_EINVAL, "U_dev and totals_dev must live on one device");
+            device = at.device;
+        }
+    }
+    if (device >= STATIC_TOTALS_MAX_DEVICES) return fail(nullptr, HYDRO_EINVAL, "device ordinal beyond 63");
+    DeviceGuard guard(device);
+    int current = -1;
+    if (cudaGetDevice(&current) != cudaSuccess || current != device)
+        return fail(nullptr, HYDRO_ECUDA, "hydro_conserved_totals_static: could not make the buffers' device current");
+    double *part = nullptr;
+    {   // set-up, on the first call that sees this device (it may load the module there: keep it out of a capture)
+        std::lock_guard<std::mutex> lock(g_static_mutex);
+        if (!g_static_partials_addr[device]) {
+            double *addr = nullptr;
+            const cudaError_t e = cudaGetSymbolAddress((void **)&addr, g_static_partials);
+            if (e != cudaSuccess || !addr) {
+                cudaGetLastError();
+                return fail(nullptr, HYDRO_ECUDA, std::string("hydro_conserved_totals_static: cudaGetSymbolAddress: ") +
+                                                      cudaGetErrorString(e));
+            }
+            g_static_partials_addr[device] = addr;
+        }
+        part = g_static_partials_addr[device];
+    }
+    // the same launch geometry as hydro_conserved_totals, hence the same reduction tree and the same bits
+    const long long nrows = (long long)g.nb[1] * g.nb[2] * g.nboxes;
+    long long blocks = (nrows + 7) / 8;
+    if (blocks > RED_BLOCKS) blocks = RED_BLOCKS;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // Pass 1 writes partial (component, block) for every block < blocks and every component < nflux; pass 2 reads
+    // exactly those.  Whatever an earlier call left in the array is therefore never read, and nothing is cleared.
+    k_totals_partial<<<dim3((unsigned)blocks, g.nflux), 256, 0, st>>>(g, (const double *)U_dev, part);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        k_totals_final<<<g.nflux, 32, 0, st>>>(g, part, (int)blocks, (double *)totals_dev);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess)
+        return fail(nullptr, HYDRO_ECUDA, std::string("hydro_conserved_totals_static: ") + cudaGetErrorString(e));
+    return HYDRO_OK;
+}
