@@ -70,13 +70,14 @@ def exchange_dim(dim, nbrs, pack, unpack, sendrecv):
     """One dimension of the halo exchange of one rank.  pack(dim, side) -> buffer of my valid layers next to
     `side`; unpack(dim, side, buffer) fills my ghost layers beyond `side`; sendrecv([(send buffer, dst rank, tag)],
     [(src rank, tag)]) -> received buffers in the order of the second list."""
-    sends, recvs, sides = [], [], []
-    for side, dst, _ in exchange_plan(nbrs, dim):
-        # tag = the side of the RECEIVER the message is for, so that two messages between the same pair of ranks
-        # (a dimension cut in two with periodic wrap) cannot be confused
-        sends.append((pack(dim, side), dst, 2 * dim + (1 - side)))
-        recvs.append((dst, 2 * dim + side))
-        sides.append(side)
+    plan = exchange_plan(nbrs, dim)
+    # Sends go out low side first.  A dimension cut in two with periodic wrap has BOTH messages of a rank going to
+    # the same peer; NCCL ignores tags and pairs the sends and receives of two ranks in posting order, so the
+    # receives are posted in the order of the peer's sends: its low-side message fills MY high ghosts, hence high
+    # side first.  The tag (the side of the RECEIVER the message is for) says the same to backends that honour tags.
+    sends = [(pack(dim, side), dst, 2 * dim + (1 - side)) for side, dst, _ in plan]
+    sides = [side for side, _, _ in reversed(plan)]
+    recvs = [(nbrs[(dim, side)], 2 * dim + side) for side in sides]
     for side, buf in zip(sides, sendrecv(sends, recvs)):
         unpack(dim, side, buf)
 

@@ -34,6 +34,44 @@ def test_local_params_and_neighbours():
     assert [S.proc_rank(S.proc_coords(r, (2, 3, 2)), (2, 3, 2)) for r in range(12)] == list(range(12))
 
 
+@pytest.mark.parametrize("pgrid,periodic", [((2, 1, 1), True), ((2, 2, 2), True), ((3, 1, 2), True), ((2, 1, 4), False)])
+def test_exchange_matches_by_posting_order_alone(pgrid, periodic):
+    """ProcessGroupNCCL ignores P2P tags: between two ranks the n-th send meets the n-th receive.  Model exactly
+    that (one FIFO per ordered pair of ranks, tags dropped) and run exchange_dim for every rank of the grid: the
+    ghost layers beyond my `side` must come from my neighbour's OPPOSITE side, also where a periodic dimension is cut
+    in two and both of a rank's messages go to the same peer."""
+    wl = W.config(5, ndom=(96, 32, 64), nbox=(16, 16, 16))
+    params = dict(wl.params)
+    if not periodic:
+        params["bc_lo"], params["bc_hi"] = [1, 1, 1], [1, 1, 1]
+    world = pgrid[0] * pgrid[1] * pgrid[2]
+    nbrs = [S.local_params(params, pgrid, r)[1] for r in range(world)]
+    for dim in range(3):
+        fifo = {}
+
+        def post(rank):          # pass 1: every rank posts its sends (payload = who packed it, from which side)
+            def sendrecv(sends, recvs):
+                for buf, dst, _tag in sends:
+                    fifo.setdefault((rank, dst), []).append(buf)
+                return [None] * len(recvs)
+            return sendrecv
+
+        def match(rank):         # pass 2: the same posting order again, receives served from the FIFOs
+            def sendrecv(sends, recvs):
+                return [fifo[(src, rank)].pop(0) for src, _tag in recvs]
+            return sendrecv
+
+        for r in range(world):
+            S.exchange_dim(dim, nbrs[r], lambda d, s, r=r: (r, s), lambda d, s, buf: None, post(r))
+        got = {}
+        for r in range(world):
+            S.exchange_dim(dim, nbrs[r], lambda d, s, r=r: (r, s),
+                           lambda d, s, buf, r=r: got.__setitem__((r, s), buf), match(r))
+        assert all(not q for q in fifo.values())
+        want = {(r, s): (nbrs[r][(dim, s)], 1 - s) for r in range(world) for s in (0, 1) if (dim, s) in nbrs[r]}
+        assert got == want
+
+
 # ---- numpy stand-ins of hydro_pack_halo / hydro_unpack_halo on a (boxes, nvar, nt2, nt1, nt0) state --------------
 def np_pack(U, wl, dim, side):
     """the ng valid layers next to `side` of dimension dim of the boxes on that face, full padded extent elsewhere"""
