@@ -371,8 +371,10 @@ void launch_energy_ring(hydro_handle h, const SweepArgs &a, dim3 grid, const Rin
     kern<<<grid, BS, sm, h->stream>>>(h->g, a, tm);
 }
 
+// The three launchers below pick a kernel instance by the species per thread; they return false (and launch
+// nothing) when no instance exists for that count, which the caller turns into HYDRO_EINVAL.
 template <int DIR, bool FINAL, int STAGE>
-void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, int state)
+bool launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, int state)
 {
     RingMaps tm;
     tm.a = h->maps[state][DIR - 1][1];
@@ -386,13 +388,16 @@ void launch_species_ring(hydro_handle h, const SweepArgs &a, int ns, dim3 grid, 
         break;
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
-        default: break;
+        default: return false;
     }
+    return true;
 }
 
-// all species groups of a direction in ONE launch (k_march_species_groups): nsa = species of the larger groups
+// all species groups of a direction in ONE launch (k_march_species_groups): nsa = species of the larger groups, >= 2
+// (with one species per group there is no rho / F_rho row to share that a plain launch per group would not also
+// find in L2, and no instance is built for it: sweep_dir launches those groups one by one)
 template <int DIR, bool FINAL, int STAGE>
-void launch_species_groups(hydro_handle h, const SweepArgs &a, int nsa, dim3 grid, int state)
+bool launch_species_groups(hydro_handle h, const SweepArgs &a, int nsa, dim3 grid, int state)
 {
     RingMaps tm;
     tm.a = h->maps[state][DIR - 1][1];
@@ -412,8 +417,9 @@ void launch_species_groups(hydro_handle h, const SweepArgs &a, int nsa, dim3 gri
         break;
         CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
-        default: break;
+        default: return false;
     }
+    return true;
 }
 
 template <int DIR, bool FINAL, int STAGE, bool FLAT, bool EVOLVE>
@@ -431,14 +437,15 @@ void launch_hydro_ring(hydro_handle h, const SweepArgs &a, dim3 grid, int state)
 }
 
 template <int DIR, bool FINAL, int STAGE>
-void launch_species(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
+bool launch_species(hydro_handle h, const SweepArgs &a, int ns, dim3 grid)
 {
     switch (ns) {
 #define CASE(N) case N: k_sweep_species<DIR, FINAL, STAGE, N, BS><<<grid, BS, 0, h->stream>>>(h->g, a); break;
         CASE(1) CASE(2) CASE(3) CASE(4) CASE(5)
 #undef CASE
-        default: break;
+        default: return false;
     }
+    return true;
 }
 
 template <int DIR, bool FINAL, int STAGE>
@@ -469,15 +476,18 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
     int rc = check_launch(h, "k_sweep_hydro", DIR == 1 ? K_HYDRO_Y : K_HYDRO_Z);
     if (rc) return rc;
     const int ngroups = g.nspec > 0 ? (g.nspec + h->ns_max - 1) / h->ns_max : 0;
-    if (ring && ngroups >= 2 && (h->kn.species_one_launch & (DIR == 1 ? 1 : 2)) && (long long)grid.x * ngroups <= 2147483647LL) {
+    const int nsa = ngroups > 0 ? (g.nspec + ngroups - 1) / ngroups : 0;   // species of the larger groups
+    if (ring && ngroups >= 2 && nsa >= 2 && (h->kn.species_one_launch & (DIR == 1 ? 1 : 2)) &&
+        (long long)grid.x * ngroups <= 2147483647LL) {
         // every group in one launch: sibling CTAs share their rho and F_rho rows through L2
-        const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
+        const int rem = g.nspec % ngroups;
         a.sbase = 0;
         a.lacc_shift = 0;
         a.ngroups = ngroups;
         a.n_hi = rem > 0 ? rem : ngroups;
         prof_begin(h);
-        launch_species_groups<DIR, FINAL, STAGE>(h, a, rem > 0 ? base + 1 : base, grid, state);
+        if (!launch_species_groups<DIR, FINAL, STAGE>(h, a, nsa, grid, state))
+            return fail(h, HYDRO_EINVAL, "no k_march_species_groups instance for " + std::to_string(nsa) + " species per thread");
         if ((rc = check_launch(h, "k_march_species_groups", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
     } else if (g.nspec > 0) {
         const int base = g.nspec / ngroups, rem = g.nspec % ngroups;
@@ -487,8 +497,9 @@ int sweep_dir(hydro_handle h, SweepArgs a, int state)
             a.sbase = s0;
             a.lacc_shift = 0;
             prof_begin(h);
-            if (ring) launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid, state);
-            else launch_species<DIR, FINAL, STAGE>(h, a, ns, grid);
+            if (!(ring ? launch_species_ring<DIR, FINAL, STAGE>(h, a, ns, grid, state)
+                       : launch_species<DIR, FINAL, STAGE>(h, a, ns, grid)))
+                return fail(h, HYDRO_EINVAL, "no species sweep instance for " + std::to_string(ns) + " species per thread");
             if ((rc = check_launch(h, "k_sweep_species", DIR == 1 ? K_SPECIES_Y : K_SPECIES_Z))) return rc;
             s0 += ns;
         }
@@ -566,7 +577,7 @@ int xmarch_stage(hydro_handle h, int state, double *Lacc, double *FX)
                 case 3: launch_xmarch_species_n<3>(h, xa, sgrid, tm); break;
                 case 4: launch_xmarch_species_n<4>(h, xa, sgrid, tm); break;
                 case 5: launch_xmarch_species_n<5>(h, xa, sgrid, tm); break;
-                default: break;
+                default: return fail(h, HYDRO_EINVAL, "no k_xmarch_species instance for " + std::to_string(ns) + " species per thread");
             }
             int rc = check_launch(h, "k_xmarch_species", K_SWEEP_X);
             if (rc) return rc;

@@ -519,3 +519,32 @@ def test_species_groups_in_one_launch_change_no_bit(name, monkeypatch):
         h.hydro_step(3)
         states.append(h.U0.clone())
     assert all(torch.equal(states[0], s) for s in states[1:])
+
+
+@pytest.mark.parametrize("name", ["cfg5_scaling_small", "cfg3_periodic_small", "cfg3_one_species_odd_box"])
+def test_species_per_thread_1_to_5_change_no_bit(name, monkeypatch):
+    """HYDRO_NSMAX (include/hydro.h, 1..5 species per thread and launch): every value gives the state of the default
+    bit for bit, with the species groups launched together where that exists (groups of >= 2 species) and one by
+    one -- a group size without a kernel instance must not be dropped silently -- and the default matches the oracle.
+    13 species (ring kernels), 3 species, and 1 species on an odd box (plain-load kernels)."""
+    import torch
+    from paper_2007_05218_b200.binding import Hydro
+    wl = CASES[name]()
+    U0 = W.initial_state(wl)
+    states = {}
+    for one_launch in ("3", "0"):
+        monkeypatch.setenv("HYDRO_SPECIES_ONE_LAUNCH", one_launch)
+        for nsmax in (5, 1, 2, 3, 4):
+            monkeypatch.setenv("HYDRO_NSMAX", str(nsmax))         # read once per hydro_init
+            h = Hydro(wl.params)
+            assert h.hydro_query(3) == nsmax
+            h.upload(U0, 0)
+            h.hydro_step(2)
+            states[(one_launch, nsmax)] = h.U0.clone()
+    ref = states[("3", 5)]
+    assert all(torch.equal(ref, s) for s in states.values()), [k for k, s in states.items() if not torch.equal(ref, s)]
+    p = O.make_params(wl.params)
+    Uo, Uo1 = U0.copy(), np.zeros_like(U0)
+    O.step(p, Uo, Uo1); O.step(p, Uo, Uo1)
+    e = rel_err(wl, ref.cpu().numpy().reshape(U0.shape), Uo)
+    assert np.all(e <= 1e-11), e
