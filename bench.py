@@ -180,7 +180,8 @@ def oracle_sample(steps, warmup, n=256, threads=None):
     same index-based generator (13 species, periodic, CFL 0.4) in 64^3 boxes, on `threads` host threads
     (None = all the cores OpenMP sees; the loop over boxes is the only parallel loop)."""
     from oracle import oracle_binding as O
-    wl = W.config(5, ndom=(n, n, n), nbox=(64, 64, 64))
+    nb = 64 if n >= 256 else 32           # at least 64 boxes: the loop over boxes is what keeps the cores busy
+    wl = W.config(5, ndom=(n, n, n), nbox=(nb, nb, nb))
     U0 = W.initial_state(wl, threads=8)
     U1 = np.zeros_like(U0)
     p = O.make_params(wl.params)
@@ -194,9 +195,9 @@ def oracle_sample(steps, warmup, n=256, threads=None):
         O.step(p, U0, U1)
     el = time.perf_counter() - t0
     O.set_threads(all_threads)
-    return {"value": wl.zones * steps / el, "unit": UNIT, "cores": used, "kind": "oracle",
-            "sample": f"config-5 recipe at {n}^3 (13 species, {wl.nboxes} boxes of 64^3), {steps} RK2 steps, "
-                      f"{used} thread(s) over boxes, {el:.1f} s"}, el / steps * 1e3, wl
+    return {"value": wl.zones * steps / el, "unit": UNIT, "cores": used, "cores_available": all_threads, "kind": "oracle",
+            "sample": f"config-5 recipe at {n}^3 (13 species, {wl.nboxes} boxes of {nb}^3), {steps} RK2 steps, "
+                      f"{used} of {all_threads} thread(s) over boxes, {el:.1f} s"}, el / steps * 1e3, wl
 
 
 def workload_config(wl, n_cfg):
@@ -212,8 +213,9 @@ def workload_config(wl, n_cfg):
 def run_reference(args, rank):
     """There is no reference implementation (paper text only): this arm times the CPU oracle, as it stands, on
     this box's host cores.  `config` is the workload of our arm (the metric is a rate per zone); a STEP of this
-    arm is one RK2 step of a BOUNDED SAMPLE of it -- the 256^3 instance of the same index-based recipe (one eighth
-    of the zones, about 6 s on 16 cores; 128^3 when more than 24 steps are asked for) -- and `config.sample`,
+    arm is one RK2 step of a BOUNDED SAMPLE of it -- the 256^3 instance of the same index-based recipe in 64^3 boxes
+    (one eighth of the zones, about 6 s on 16 cores), or the 128^3 instance in 32^3 boxes when more than 24 steps are
+    asked for; 64 boxes either way, so every core has work -- and `config.zones`, `config.sample`,
     `cpu_baseline.sample` and `ms_per_step` describe that sample, so that K + W steps end within a few minutes."""
     if rank != 0:
         return
@@ -223,6 +225,9 @@ def run_reference(args, rank):
     cb.update(host_info())
     cfg = workload_config(W.config(args.config), args.config)
     cfg["l2_policy"] = "n/a (host)"
+    cfg["full_workload_zones"] = cfg["zones"]
+    cfg["zones"] = wl.zones                      # what a step of THIS arm advances
+    cfg["state_gb"] = round(wl.state_bytes / 1e9, 3)
     cfg["sample"] = {"workload": workload_config(wl, args.config)["workload"], "zones": wl.zones,
                      "state_gb": round(wl.state_bytes / 1e9, 3),
                      "why": "the oracle needs about 50 s per RK2 step of the 512^3 state on 16 cores; its rate per zone "
