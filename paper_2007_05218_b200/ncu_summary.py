@@ -21,18 +21,37 @@ CSRC = os.path.join(HERE, "csrc")
 N_SM = 148
 
 
-# the kernel sources of the RK2 path's default launches (the classes of hydro_profile_read 0..8)
-PATH_SOURCES = ["flatten.cuh", "ghost_reduce.cuh", "hydro_device.cuh", "march_ring.cuh", "sweep_x.cuh", "sweep_xc.cuh", "sweep_yz.cuh"]
+# what decides the kernels of the RK2 path's default launches (the classes of hydro_profile_read 0..8) and how they
+# are launched: the kernel sources, and hydro_api.cu (ring depths, CTA sizes, launch bounds, species grouping, grids)
+PATH_SOURCES = ["flatten.cuh", "ghost_reduce.cuh", "hydro_device.cuh", "march_ring.cuh", "sweep_x.cuh", "sweep_xc.cuh", "sweep_yz.cuh",
+                "hydro_api.cu"]
+# the run-time switches of include/hydro.h: each selects another code path, hence other per-launch traffic
+KNOBS = ["HYDRO_RING", "HYDRO_XCHUNK", "HYDRO_XMARCH", "HYDRO_SEGLEN", "HYDRO_NSMAX", "HYDRO_SPECIES_ONE_LAUNCH", "HYDRO_FUSE_DT",
+         "HYDRO_SPLIT_GHOSTS", "HYDRO_FILL_MONOLITHIC"]
+
+
+def build_flags() -> str:
+    """The flags the library in the tree was built with (the stamp build.py writes next to it), else what a build
+    started now would use."""
+    stamp = os.path.join(HERE, "libhydro_b200.so.flags")
+    if os.path.exists(stamp):
+        return open(stamp).read()
+    return "fmad=%d extra=%s" % (int(os.environ.get("HYDRO_FMAD", "1") != "0"), os.environ.get("HYDRO_NVCC_EXTRA", ""))
 
 
 def source_sha() -> str:
-    """SHA-256 over the kernel sources of the RK2 path (names and contents): a capture is trusted while the
-    kernels it measured are the kernels that run.  The optional paths (march_x.cuh, ctu.cuh) and the host code
+    """SHA-256 over everything that decides which kernels of the RK2 path run and what they move: the kernel
+    sources and hydro_api.cu (names and contents), the build flags of the library, and the values of the run-time
+    switches in this environment.  A capture is trusted only while all of that is what it was measured with; run
+    the summary in the environment (switches, build) of the capture.  The optional paths (march_x.cuh, ctu.cuh)
     are not part of it."""
     h = hashlib.sha256()
     for name in PATH_SOURCES:
         h.update(name.encode())
         h.update(open(os.path.join(CSRC, name), "rb").read())
+    h.update(("flags:" + build_flags()).encode())
+    for k in KNOBS:
+        h.update(("%s=%s;" % (k, os.environ.get(k, ""))).encode())
     return h.hexdigest()
 
 

@@ -49,3 +49,24 @@ def test_two_rank_aggregation_gloo():
         assert ms == 15.0                               # max over ranks, on every rank
         assert value == pytest.approx(2 * 1000 * 3 / 0.015)
         assert out == ""
+
+
+def test_capture_hash_covers_host_code_flags_and_switches(monkeypatch):
+    """bench.py trusts the per-launch DRAM bytes of profiles/traffic.json only while ncu_summary.source_sha() is
+    unchanged: the hash must move with hydro_api.cu (ring depths, grids, species grouping), with the build flags and
+    with every run-time switch of include/hydro.h."""
+    from paper_2007_05218_b200 import ncu_summary as N
+    hdr = open(os.path.join(ROOT, "include", "hydro.h")).read()
+    import re
+    assert set(re.findall(r"^ \*   (HYDRO_[A-Z_]+)=", hdr, flags=re.M)) == set(N.KNOBS)
+    assert "hydro_api.cu" in N.PATH_SOURCES
+    for k in N.KNOBS:
+        monkeypatch.delenv(k, raising=False)
+    base = N.source_sha()
+    for k in N.KNOBS:
+        monkeypatch.setenv(k, "2")
+        assert N.source_sha() != base, k
+        monkeypatch.delenv(k)
+    assert N.source_sha() == base
+    monkeypatch.setattr(N, "build_flags", lambda: "fmad=0 extra=")
+    assert N.source_sha() != base
