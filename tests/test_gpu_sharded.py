@@ -66,6 +66,20 @@ def test_sharded_equals_unsharded_bit_for_bit(name, make, pgrid):
     tr, ts = np.array(ref.hydro_conserved_totals(0)), np.array(sh.totals())
     scale = np.abs(Gr).sum(axis=(1, 2, 3))[[0, 1, 2, 3, 4] + list(range(6, wl.nvar))] * np.prod(wl.dx)
     assert np.all(np.abs(tr - ts) <= 1e-13 * scale)
+    # and the loop is closed to the oracle, not only to the unsharded CUDA run: the state gathered from the shards
+    # against three oracle steps of the unsharded domain (north_star's multi-step bound)
+    from oracle import oracle_binding as O
+    from parity_util import rel_err
+    p = O.make_params(wl.params)
+    Uo, U1 = U0.copy(), np.zeros_like(U0)
+    for _ in range(3):
+        O.step(p, Uo, U1)
+    Gs = np.empty_like(Gr)
+    for r, sl in shard_blocks(wl, pgrid):
+        s = sh.shards[r]
+        Gs[sl] = W.gather_valid(s.wl, s.h.download(0).reshape(s.wl.state_shape))
+    e = rel_err(wl, W.scatter_valid(wl, Gs, ghost_value=np.nan), Uo)
+    assert np.all(e <= 1e-10), e
 
 
 def test_a_shard_refuses_hydro_step_and_reports_halo_sizes():
