@@ -186,6 +186,8 @@ def oracle_sample(steps, warmup, n=256, threads=None):
     U1 = np.zeros_like(U0)
     p = O.make_params(wl.params)
     all_threads = O.max_threads()
+    if "TORCHELASTIC_RUN_ID" in os.environ:      # torchrun sets OMP_NUM_THREADS=1 for its ranks; rank 0 alone works here
+        all_threads = max(all_threads, len(os.sched_getaffinity(0)))
     O.set_threads(threads or all_threads)
     used = min(threads or all_threads, wl.nboxes)
     for _ in range(warmup):
@@ -477,6 +479,32 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def dry_run(args, rank, world, local_rank):
+    """--dry-run: everything about the launch that needs no GPU.  Every rank joins a gloo process group, the ranks
+    are gathered and the per-rank times go through the same reduce_max / job_value as the timed run; rank 0 prints
+    the line's skeleton (no value is a measurement)."""
+    import torch
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    seen = [rank]
+    if world > 1:
+        t = torch.zeros(world, dtype=torch.int64)
+        t[rank] = local_rank + 1
+        dist.all_reduce(t)
+        seen = [r for r in range(world) if t[r] > 0]
+    ms = reduce_max(1.0 + rank, world)
+    wl = W.config(args.config)
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "impl": args.impl, "metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world,
+                          "ranks": seen, "steps": args.steps, "warmup": args.warmup, "ms_per_step": None,
+                          "max_over_ranks_check_ms": ms, "replica_aggregate_check": job_value(wl.zones, 1, 1e3, world) / wl.zones,
+                          "higher_is_better": True, "scaling": "weak", "dtype": "f64", "data": "synthetic",
+                          "config": workload_config(wl, args.config)}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -489,10 +517,24 @@ def main():
     ap.add_argument("--ctu", action="store_true", help="time the CTU update O12 (hydro_ctu_step) instead of the RK2 path")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--dry-run", action="store_true",
+                    help="launch check without CUDA: start the ranks, form the process group over gloo, print the line's skeleton")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # a plain `python bench.py --gpus N`: nobody has started the ranks, so start them here -- one process per
+        # GPU under torch.distributed.run, exactly the launch the driver uses -- and hand back its exit code
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+        raise SystemExit(subprocess.run(cmd).returncode)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.dry_run:
+        return dry_run(args, rank, world, local_rank)
     if args.impl == "reference":
         run_reference(args, rank)
     else:

@@ -70,3 +70,24 @@ def test_capture_hash_covers_host_code_flags_and_switches(monkeypatch):
     assert N.source_sha() == base
     monkeypatch.setattr(N, "build_flags", lambda: "fmad=0 extra=")
     assert N.source_sha() != base
+
+
+def test_plain_gpus_2_invocation_starts_two_ranks():
+    """`python bench.py --gpus 2` with no launcher around it must itself start one rank per GPU (it used to run ONE
+    replica and print n_gpus 1).  --dry-run stops before CUDA: the ranks join a gloo group and rank 0 prints the
+    line's skeleton, which must show both ranks, the max over ranks and the whole-job aggregate."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [json.loads(l) for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, res.stdout                     # rank 0 alone prints
+    line = lines[0]
+    assert line["dry_run"] is True and line["n_gpus"] == 2 and line["ranks"] == [0, 1]
+    assert line["max_over_ranks_check_ms"] == 2.0          # ranks report 1.0 and 2.0: the slower one counts
+    assert line["replica_aggregate_check"] == 2.0          # value = the zones of BOTH replicas over that time
+    one = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--dry-run"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert one.returncode == 0 and json.loads(one.stdout.splitlines()[-1])["n_gpus"] == 1
