@@ -69,6 +69,11 @@ typedef struct {
     int32_t flatten;            /* 0: off; 1: PPM shock flattening O10, needs ng >= 4 */
     int32_t evolve_eint;        /* 0: rho*e re-synchronised from rho*E after every stage; 1: evolved rho*e with a
                                    dual-energy switch, O11 */
+    double  dx[3];              /* 0: zone width = (prob_hi - prob_lo)/ndom.  > 0: THIS zone width, and prob_lo / prob_hi
+                                   only have to be ordered.  For a shard or a refined patch, whose extent is a piece of
+                                   another handle's domain: the quotient of the piece's own extent can differ from the
+                                   parent's zone width by an ulp (non-dyadic spacings), and then the piece no longer gives
+                                   the parent's bits.  The drivers sharded.py / amr.py pass the parent's dx (/ ratio) */
 } hydro_params;
 
 typedef struct hydro_ctx *hydro_handle;

@@ -19,8 +19,11 @@ BC_EXTERNAL = 3
 def patch_params(coarse_params: dict, lo, extent, ratio: int, nbox) -> dict:
     """hydro_params of the patch covering coarse zones [lo, lo + extent) refined by `ratio`, in boxes of `nbox` fine zones."""
     p = copy.deepcopy(coarse_params)
+    p["dx"] = [0.0, 0.0, 0.0]
     for d in range(3):
-        dx = (coarse_params["prob_hi"][d] - coarse_params["prob_lo"][d]) / coarse_params["ndom"][d]
+        dx = coarse_params.get("dx", (0.0, 0.0, 0.0))[d] or \
+            (coarse_params["prob_hi"][d] - coarse_params["prob_lo"][d]) / coarse_params["ndom"][d]
+        p["dx"][d] = dx / ratio          # exactly the coarse zone width over 2 or 4, whatever the patch's own extent gives
         if lo[d] < 0 or lo[d] + extent[d] > coarse_params["ndom"][d]:
             raise ValueError("the patch must lie inside the coarse domain")
         p["ndom"][d] = ratio * extent[d]

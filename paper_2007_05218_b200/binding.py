@@ -31,6 +31,7 @@ class HydroParams(C.Structure):
         ("gamma", C.c_double), ("cfl", C.c_double), ("grav", C.c_double * 3),
         ("small_dens", C.c_double), ("small_pres", C.c_double),
         ("flatten", C.c_int32), ("evolve_eint", C.c_int32),
+        ("dx", C.c_double * 3),
     ]
 
 
@@ -45,6 +46,7 @@ def make_params(d: dict) -> HydroParams:
     p.small_dens, p.small_pres = float(d.get("small_dens", 1e-12)), float(d.get("small_pres", 1e-14))
     p.flatten = int(d.get("flatten", 0))
     p.evolve_eint = int(d.get("evolve_eint", 0))
+    p.dx = (C.c_double * 3)(*[float(x) for x in d.get("dx", (0.0, 0.0, 0.0))])
     return p
 
 

@@ -158,7 +158,8 @@ bool make_geom(const hydro_params *p, Geom &g, std::string &why)
         g.nb[d] = p->nbox[d]; g.nt[d] = p->nbox[d] + 2 * p->ng; g.NB[d] = p->ndom[d] / p->nbox[d];
         g.ndom[d] = p->ndom[d]; g.bc_lo[d] = p->bc_lo[d]; g.bc_hi[d] = p->bc_hi[d];
         g.nboxes *= g.NB[d];
-        dx[d] = (p->prob_hi[d] - p->prob_lo[d]) / p->ndom[d];
+        if (!(p->dx[d] >= 0.0) || std::isinf(p->dx[d])) { why = "dx must be 0 (derive it from the extent) or a positive finite zone width"; return false; }
+        dx[d] = p->dx[d] > 0.0 ? p->dx[d] : (p->prob_hi[d] - p->prob_lo[d]) / p->ndom[d];
         g.dxinv[d] = 1.0 / dx[d];
         g.grav[d] = p->grav[d];
     }

@@ -43,10 +43,14 @@ def local_params(params: dict, pgrid, rank: int):
         if params["ndom"][d] % params["nbox"][d] or nboxes % P:
             raise ValueError(f"dimension {d}: {nboxes} boxes cannot be cut into {P} equal blocks")
         n = params["ndom"][d] // P
-        dx = (params["prob_hi"][d] - params["prob_lo"][d]) / params["ndom"][d]
+        dx = params.get("dx", (0.0, 0.0, 0.0))[d] or (params["prob_hi"][d] - params["prob_lo"][d]) / params["ndom"][d]
         p["ndom"][d] = n
         p["prob_lo"][d] = params["prob_lo"][d] + c[d] * n * dx
         p["prob_hi"][d] = params["prob_lo"][d] + (c[d] + 1) * n * dx
+        # the zone width of the UNSHARDED domain, bit for bit: (prob_hi - prob_lo)/n of the piece is off by an ulp for
+        # a third of the non-dyadic spacings, and the shards would then differ from the unsharded run and each other
+        p["dx"] = list(p.get("dx", (0.0, 0.0, 0.0)))
+        p["dx"][d] = p["dx"][d] or dx
         if P == 1:
             continue
         periodic = params["bc_lo"][d] == 0

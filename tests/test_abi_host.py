@@ -43,8 +43,9 @@ def test_probe_library_is_separate(lib):
 
 
 def test_struct_layout_matches_header():
-    # 3+3+1+1+3+3 int32 = 56 bytes, then 3+3+1+1+3+1+1 doubles = 104 bytes, then flatten + evolve_eint
-    assert C.sizeof(B.HydroParams) == 56 + 104 + 8 and B.HydroParams.flatten.offset == 160
+    # 3+3+1+1+3+3 int32 = 56 bytes, then 3+3+1+1+3+1+1 doubles = 104 bytes, then flatten + evolve_eint, then dx[3]
+    assert C.sizeof(B.HydroParams) == 56 + 104 + 8 + 24 and B.HydroParams.flatten.offset == 160
+    assert B.HydroParams.dx.offset == 168
     assert B.HydroParams.prob_lo.offset == 56 and B.HydroParams.small_pres.offset == 152
 
 

@@ -10,7 +10,16 @@ from paper_2007_05218_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
+def nondyadic():
+    """48 zones over [0.1, 1.3]: the zone width of half the domain, derived from the half's own extent, differs from
+    the unsharded zone width by an ulp; the shards must use the unsharded one (hydro_params.dx)."""
+    wl = W.config(5, ndom=(48, 24, 24), nbox=(12, 12, 12), nspec=2)
+    wl.params["prob_lo"], wl.params["prob_hi"] = [0.1, 0.1, 0.1], [1.3, 0.7, 0.7]
+    return wl
+
+
 CASES = [
+    ("cfg5 periodic on a non-dyadic domain, cut in x and y", nondyadic, (2, 2, 1)),
     ("cfg5 periodic, cut in x", lambda: W.config(5, ndom=(64, 32, 32), nbox=(16, 16, 16), nspec=3), (2, 1, 1)),
     ("cfg5 periodic, cut in z (4 slabs)", lambda: W.config(5, ndom=(32, 32, 64), nbox=(16, 16, 16), nspec=2), (1, 1, 4)),
     ("cfg5 periodic, 2x2x2 blocks", lambda: W.config(5, ndom=(64, 64, 64), nbox=(16, 16, 16), nspec=13), (2, 2, 2)),

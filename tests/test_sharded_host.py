@@ -72,6 +72,30 @@ def test_exchange_matches_by_posting_order_alone(pgrid, periodic):
         assert got == want
 
 
+def test_shards_carry_the_global_zone_width_exactly():
+    """(prob_hi - prob_lo)/ndom of a piece of a non-dyadic domain is off by an ulp in many cases (48 zones over
+    [0.1, 1.3] cut in two is one), and a shard with another dx no longer gives the bits of the unsharded run:
+    local_params hands every shard the unsharded zone width in hydro_params.dx, which the library then uses instead
+    of the quotient.  The library rejects a negative or non-finite dx."""
+    from paper_2007_05218_b200 import binding as B
+    from paper_2007_05218_b200 import build as build_mod
+    wl = W.config(5, ndom=(48, 24, 24), nbox=(12, 12, 12), nspec=2)
+    wl.params["prob_lo"], wl.params["prob_hi"] = [0.1, 0.1, 0.1], [1.3, 0.7, 0.7]
+    dx = [(wl.params["prob_hi"][d] - wl.params["prob_lo"][d]) / wl.params["ndom"][d] for d in range(3)]
+    off = 0
+    for r in range(4):
+        p, _ = S.local_params(wl.params, (2, 2, 1), r)
+        assert p["dx"] == dx                                                          # all three, cut or not
+        off += (p["prob_hi"][0] - p["prob_lo"][0]) / p["ndom"][0] != dx[0]
+        assert B.make_params(p).dx[0] == dx[0]
+    assert off > 0                     # the case is one where the piece's own quotient would have been wrong
+    build_mod.build()
+    assert B.hydro_state_bytes(B.make_params(p)) > 0
+    for bad in (-1.0, float("inf"), float("nan")):
+        q = dict(p, dx=[bad, 0.0, 0.0])
+        assert B.hydro_state_bytes(B.make_params(q)) == 0
+
+
 # ---- numpy stand-ins of hydro_pack_halo / hydro_unpack_halo on a (boxes, nvar, nt2, nt1, nt0) state --------------
 def np_pack(U, wl, dim, side):
     """the ng valid layers next to `side` of dimension dim of the boxes on that face, full padded extent elsewhere"""
