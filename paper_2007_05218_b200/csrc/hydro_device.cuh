@@ -46,7 +46,7 @@ __device__ __forceinline__ double ppm_slope(double am, double a, double ap)
     const double dp = ap - a;
     const double dm = a - am;
     const double dc = HALF * (ap - am);
-    const double lim = dmin(fabs(dc), dmin(2.0 * fabs(dp), 2.0 * fabs(dm)));
+    const double lim = dmin(fabs(dc), 2.0 * dmin(fabs(dp), fabs(dm)));   // = min(|dc|, 2|dp|, 2|dm|) exactly (x2 is exact)
     return (dp * dm > 0.0) ? copysign(lim, dc) : 0.0;
 }
 
@@ -57,8 +57,27 @@ __device__ __forceinline__ double ppm_edge(double a, double ap, double s, double
 }
 
 // ---- O4: monotonised parabola edges of one zone (CW84 1.10) --------------------------
+// HYDRO_PPM_DIFF (default build only; the strict build keeps the definitional form below so that it stays equal to
+// the oracle bit for bit): the same case analysis written on the edge differences dl = a - el, dr = er - a.  With
+// d = dl + dr and a - (el + er)/2 = (dl - dr)/2, CW84's overshoot test d*(a - (el+er)/2) > d^2/6 is |dl| > 2|dr|
+// (dl, dr of one sign, else the zone is flat), and 3a - 2er = a - 2dr: 7 FP64 operations instead of 13, the same
+// three compares and four selects.  The two forms differ by rounding only (both branches are continuous).
+#ifndef HYDRO_PPM_DIFF
+#define HYDRO_PPM_DIFF 1
+#endif
 __device__ __forceinline__ void ppm_mono(double el, double er, double a, double& aL, double& aR)
 {
+#if !defined(HYDRO_STRICT) && HYDRO_PPM_DIFF
+    const double dl = a - el, dr = er - a;
+    const bool flat = dr * dl <= 0.0;
+    const double dl2 = dl + dl, dr2 = dr + dr;
+    const bool over_l = fabs(dl) > fabs(dr2);
+    const bool over_r = fabs(dr) > fabs(dl2);
+    const double l1 = over_l ? a - dr2 : el;
+    const double r1 = over_r ? a + dl2 : er;
+    aL = flat ? a : l1;
+    aR = flat ? a : r1;
+#else
     // branch-free: every candidate is evaluated and the CW84 (1.10) cases pick among them, so
     // the five variables of a zone stay in one basic block and interleave in the FP64 pipe.
     // The selected values are the same expressions as in the if/else form of the definition.
@@ -80,6 +99,7 @@ __device__ __forceinline__ void ppm_mono(double el, double er, double a, double&
     const double r1 = over_r ? 3.0 * a - 2.0 * el : er;
     aL = flat ? a : l1;
     aR = flat ? a : r1;
+#endif
 #endif
 }
 
